@@ -1,0 +1,540 @@
+// ============================================================================================
+//  hydro_oracle.cpp  --  TEST INFRASTRUCTURE, NOT PRODUCT.
+//
+//  Plain, slow, scalar fp64 CPU implementation of the hot path of arxiv 1511.02137
+//  (ideal relativistic hydrodynamics with a jet source on a 3-D Cartesian grid):
+//     d_mu T^{mu nu} = S^nu                            PAPER.md:17-19  (eq. 1)
+//     S^nu = sum_jets (-dE/dt, -dM/dt) delta^3(x-x_jet) PAPER.md:21-23  (eq. 2)
+//     -dE/dx = k_rad (C_R/C_F) T^3 x + k_coll (C_R/C_F) T^2   PAPER.md:27-31 (eq. 3)
+//     "7th order WENO", "third order Runge-Kutta"
+//     dx, dt, grid, EOS p = e/3
+//  Everything the paper leaves open follows the readings R1-R14 listed in DESIGN.md
+//  (taken from SURVEY.md 8(c)); the steps are numbered O1..O9 as there.
+//
+//  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may
+//  load this library.  It shares NO code, header, table or helper with the CUDA path under
+//  paper_1511_02137_b200/csrc and include/.  No blocking, fusion or reordering beyond what the
+//  algorithm states: per stage, primitives for every cell, then for every direction, every
+//  grid line, every interface the eight-cell window is gathered and reconstructed.
+//  `#pragma omp parallel for` over independent grid lines / cells is the only concession
+//  (each cell's arithmetic is unchanged; the only reduction is an exact max / integer sum).
+//
+//  Pins (tests/test_oracle_*.py, -m "not gpu"): P1 con2prim round trip, P2 uniform state
+//  bitwise, P3 WENO7 exactness/order/weights, P4 exact Riemann solution, P5 discrete
+//  conservation + jet budget, P6 mirror symmetry, P7 dimensional embedding/permutation,
+//  P8 source-law values.  The readings R2,R3,R4,R7,R9 themselves cannot be pinned by any
+//  number printed in the paper (it prints none): "parity unpinned against the paper" for those
+//  choices; they are fixed by DESIGN.md only.
+//
+//  Build: g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC hydro_oracle.cpp -o liboracle.so
+// ============================================================================================
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+#include <algorithm>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+// ---------------------------------------------------------------- operation-counting number
+// Used only by oracle_count_flops(): the same templated per-cell routines run on this type and
+// every +,-,*,/ and sqrt is counted as one flop ("FMA = 2, add/mul/div/sqrt = 1").
+struct Counted {
+    double v;
+    static long long ops;
+    Counted() : v(0.0) {}
+    Counted(double x) : v(x) {}
+};
+long long Counted::ops = 0;
+inline Counted operator+(Counted a, Counted b) { ++Counted::ops; return Counted(a.v + b.v); }
+inline Counted operator-(Counted a, Counted b) { ++Counted::ops; return Counted(a.v - b.v); }
+inline Counted operator*(Counted a, Counted b) { ++Counted::ops; return Counted(a.v * b.v); }
+inline Counted operator/(Counted a, Counted b) { ++Counted::ops; return Counted(a.v / b.v); }
+inline Counted operator-(Counted a) { return Counted(-a.v); }               // sign flip: free
+inline bool operator>(Counted a, Counted b) { return a.v > b.v; }
+inline bool operator<(Counted a, Counted b) { return a.v < b.v; }
+inline Counted rsqrt_(Counted a) { ++Counted::ops; return Counted(std::sqrt(a.v)); }
+inline double rsqrt_(double a) { return std::sqrt(a); }
+inline Counted rabs_(Counted a) { return Counted(std::fabs(a.v)); }         // comparisons: free
+inline double rabs_(double a) { return std::fabs(a); }
+inline Counted rmax_(Counted a, Counted b) { return a.v > b.v ? a : b; }
+inline double rmax_(double a, double b) { return a > b ? a : b; }
+inline double val_(Counted a) { return a.v; }
+inline double val_(double a) { return a; }
+
+// ---------------------------------------------------------------- O1: constants
+const double HBARC = 0.1973269804;                     // GeV fm
+const double PI_ = 3.14159265358979323846;
+const double G_DOF = 47.5 * PI_ * PI_ / 30.0;          // e = g * hbarc * T^4  (BASELINE.json cfg 0)
+const double CS2 = 1.0 / 3.0;                          // EOS p = e/3
+
+template <class R> struct Prim { R e, p, vx, vy, vz, n; int limited; };
+
+// ---------------------------------------------------------------- O3: con2prim, p = e/3
+// eq. (1) with u^mu = gamma(1,v):  E = (e+p) gamma^2 - p,  M = (e+p) gamma^2 v
+//   => (E+p)^2 - M^2 = (E+p)(e+p)  => with p = e/3:  e^2 + 2 E e - 3 (E^2 - M^2) = 0
+//   => e = -E + sqrt(4E^2 - 3M^2) = 3 (E^2 - M^2) / (E + sqrt(4E^2 - 3M^2)).
+// Reading R9: E floored at e_floor, |M| capped at (1-delta) E; U itself is never modified.
+template <class R>
+Prim<R> con2prim(R E, R Mx, R My, R Mz, R NB, double e_floor, double delta) {
+    Prim<R> P;
+    P.limited = 0;
+    if (E < R(e_floor)) { E = R(e_floor); P.limited = 1; }
+    R M = rsqrt_(Mx * Mx + My * My + Mz * Mz);
+    R cap = R(1.0 - delta) * E;
+    if (M > cap) {
+        R sc = cap / M;
+        Mx = Mx * sc; My = My * sc; Mz = Mz * sc;
+        P.limited = 1;
+    }
+    R M2 = Mx * Mx + My * My + Mz * Mz;
+    R s = rsqrt_(R(4.0) * E * E - R(3.0) * M2);
+    P.e = R(3.0) * (E * E - M2) / (E + s);
+    P.p = P.e / R(3.0);
+    R w = E + P.p;
+    P.vx = Mx / w; P.vy = My / w; P.vz = Mz / w;
+    R v2 = P.vx * P.vx + P.vy * P.vy + P.vz * P.vz;
+    R om = R(1.0) - v2;
+    if (om < R(0.0)) om = R(0.0);
+    P.n = NB * rsqrt_(om);
+    return P;
+}
+
+// ---------------------------------------------------------------- O4: acoustic wavespeeds
+// lambda_pm^d = [ v_d (1-cs2) +- cs sqrt( (1-v^2) (1 - v^2 cs2 - v_d^2 (1-cs2)) ) ] / (1 - v^2 cs2)
+// returns max(|lambda_+|, |lambda_-|) for direction d (vd = velocity component along d).
+template <class R>
+R max_wavespeed(R vd, R v2) {
+    R cs = rsqrt_(R(CS2));
+    R rad = (R(1.0) - v2) * (R(1.0) - v2 * R(CS2) - vd * vd * R(1.0 - CS2));
+    if (rad < R(0.0)) rad = R(0.0);
+    R root = cs * rsqrt_(rad);
+    R den = R(1.0) - v2 * R(CS2);
+    R a = vd * R(1.0 - CS2);
+    R lp = (a + root) / den;
+    R lm = (a - root) / den;
+    return rmax_(rabs_(lp), rabs_(lm));
+}
+// variant of the above without recomputing sqrt(cs2) per call when counting flops is irrelevant
+
+// ---------------------------------------------------------------- O5: WENO7 (r = 4), WENO-JS
+// value at the right face i+1/2 of the centre cell `d` from a..g = phi_{i-3}..phi_{i+3}.
+// Expanded x240 smoothness indicators, one division per nonlinear weight (reading R3).
+template <class R>
+void weno7_parts(R a, R b, R c, R d, R e, R f, R g, R q[4], R beta[4]) {
+    q[0] = (R(-3.0) * a + R(13.0) * b - R(23.0) * c + R(25.0) * d) / R(12.0);
+    q[1] = (b - R(5.0) * c + R(13.0) * d + R(3.0) * e) / R(12.0);
+    q[2] = (-c + R(7.0) * d + R(7.0) * e - f) / R(12.0);
+    q[3] = (R(3.0) * d + R(13.0) * e - R(5.0) * f + g) / R(12.0);
+    beta[0] = (a * (R(547.0) * a - R(3882.0) * b + R(4642.0) * c - R(1854.0) * d)
+             + b * (R(7043.0) * b - R(17246.0) * c + R(7042.0) * d)
+             + c * (R(11003.0) * c - R(9402.0) * d)
+             + R(2107.0) * d * d) / R(240.0);
+    beta[1] = (b * (R(267.0) * b - R(1642.0) * c + R(1602.0) * d - R(494.0) * e)
+             + c * (R(2843.0) * c - R(5966.0) * d + R(1922.0) * e)
+             + d * (R(3443.0) * d - R(2522.0) * e)
+             + R(547.0) * e * e) / R(240.0);
+    beta[2] = (c * (R(547.0) * c - R(2522.0) * d + R(1922.0) * e - R(494.0) * f)
+             + d * (R(3443.0) * d - R(5966.0) * e + R(1602.0) * f)
+             + e * (R(2843.0) * e - R(1642.0) * f)
+             + R(267.0) * f * f) / R(240.0);
+    beta[3] = (d * (R(2107.0) * d - R(9402.0) * e + R(7042.0) * f - R(1854.0) * g)
+             + e * (R(11003.0) * e - R(17246.0) * f + R(4642.0) * g)
+             + f * (R(7043.0) * f - R(3882.0) * g)
+             + R(547.0) * g * g) / R(240.0);
+}
+
+const double WENO_D[4] = {1.0 / 35.0, 12.0 / 35.0, 18.0 / 35.0, 4.0 / 35.0};
+
+template <class R>
+R weno7(R a, R b, R c, R d, R e, R f, R g, double eps) {
+    R q[4], beta[4], al[4];
+    weno7_parts(a, b, c, d, e, f, g, q, beta);
+    for (int k = 0; k < 4; ++k) {
+        R t = R(eps) + beta[k];
+        al[k] = R(WENO_D[k]) / (t * t);
+    }
+    R sum = al[0] + al[1] + al[2] + al[3];
+    R num = al[0] * q[0] + al[1] * q[1] + al[2] * q[2] + al[3] * q[3];
+    return num / sum;
+}
+
+// sum-of-three-squares form of the same beta_k -- used only by the pin that
+// checks the expanded form against it.
+void weno7_beta_sos(double a, double b, double c, double d, double e, double f, double g, double beta[4]) {
+    double L1, L2, L3;
+    L1 = 44 * d - 72 * c + 36 * b - 8 * a; L2 = 2 * d - 5 * c + 4 * b - a; L3 = d - 3 * c + 3 * b - a;
+    beta[0] = L1 * L1 / 576.0 + 13.0 / 12.0 * L2 * L2 + 781.0 / 720.0 * L3 * L3;
+    L1 = 12 * d - 24 * c + 4 * b + 8 * e; L2 = c - 2 * d + e; L3 = -3 * d + 3 * c - b + e;
+    beta[1] = L1 * L1 / 576.0 + 13.0 / 12.0 * L2 * L2 + 781.0 / 720.0 * L3 * L3;
+    L1 = -12 * d - 8 * c + 24 * e - 4 * f; L2 = c - 2 * d + e; L3 = 3 * d - c - 3 * e + f;
+    beta[2] = L1 * L1 / 576.0 + 13.0 / 12.0 * L2 * L2 + 781.0 / 720.0 * L3 * L3;
+    L1 = -44 * d + 72 * e - 36 * f + 8 * g; L2 = 2 * d - 5 * e + 4 * f - g; L3 = -d + 3 * e - 3 * f + g;
+    beta[3] = L1 * L1 / 576.0 + 13.0 / 12.0 * L2 * L2 + 781.0 / 720.0 * L3 * L3;
+}
+
+// ---------------------------------------------------------------- a-3: physical flux along d
+// F^d = (M_d, M_x v_d + p delta_xd, M_y v_d + p delta_yd, M_z v_d + p delta_zd [, N_B v_d])
+template <class R>
+void phys_flux(int d, const R U[5], const Prim<R>& P, int nf, R F[5]) {
+    R vd = (d == 0) ? P.vx : (d == 1) ? P.vy : P.vz;
+    F[0] = U[1 + d];
+    F[1] = U[1] * vd; F[2] = U[2] * vd; F[3] = U[3] * vd;
+    F[1 + d] = F[1 + d] + P.p;
+    if (nf > 4) F[4] = U[4] * vd;
+}
+
+// ---------------------------------------------------------------- O6: one interface flux
+// Uw[m], Pw[m], m = 0..7  <->  cells i-3 .. i+4 along d (already clamped by the caller).
+// NOTE reading R9: fluxes use the *limited* momenta consistently?  No: O3 says only the
+// primitives are limited; U entering F^d_E = M_d and the alpha*U term is the stored U.
+template <class R>
+void interface_flux(int d, int nf, const R Uw[8][5], const Prim<R> Pw[8], R alpha, double eps, R Fhat[5]) {
+    R fp[8][5], fm[8][5];
+    for (int m = 0; m < 8; ++m) {
+        R F[5];
+        phys_flux(d, Uw[m], Pw[m], nf, F);
+        for (int q = 0; q < nf; ++q) {
+            fp[m][q] = R(0.5) * (F[q] + alpha * Uw[m][q]);
+            fm[m][q] = R(0.5) * (F[q] - alpha * Uw[m][q]);
+        }
+    }
+    for (int q = 0; q < nf; ++q) {
+        R wp = weno7(fp[0][q], fp[1][q], fp[2][q], fp[3][q], fp[4][q], fp[5][q], fp[6][q], eps);
+        R wm = weno7(fm[7][q], fm[6][q], fm[5][q], fm[4][q], fm[3][q], fm[2][q], fm[1][q], eps);
+        Fhat[q] = wp + wm;
+    }
+}
+
+// ---------------------------------------------------------------- O8: source law
+// T = (e/(g hbarc))^{1/4} [1/fm];  q = hbarc * (C_R/C_F) * (k_rad T^3 l + k_coll T^2)  [GeV/fm]
+double source_q(double e_c, double ell, double k_rad, double k_coll, double crcf) {
+    double T = std::pow(e_c / (G_DOF * HBARC), 0.25);
+    return HBARC * crcf * (k_rad * T * T * T * ell + k_coll * T * T);
+}
+
+struct Jet { double x0, y0, z0, nx, ny, nz, k_rad, k_coll, crcf; long long step_added; };
+
+// R7: deposit cell index along one axis; returns -1 if outside.
+int jet_axis_index(double x, int n, double dx) {
+    double xmin = -0.5 * n * dx;
+    double a = (x - xmin) / dx + 1.0 / 1048576.0;     // + 2^-20
+    double fl = std::floor(a);
+    if (fl < 0.0 || fl > (double)(n - 1)) return -1;
+    return (int)fl;
+}
+
+struct Oracle {
+    int nx, ny, nz, nf;
+    double dx, dt, eps, delta, e_floor;
+    long long step;                 // integer step counter; t = step*dt (O1)
+    std::vector<double> U, U1, U2, L;
+    std::vector<Prim<double> > P;
+    std::vector<Jet> jets;
+    double alpha[3];
+    long long ncap;
+    int has_nan;
+    double deposited[4];
+    double last_q[3][16];           // q per stage for up to 16 jets (for the P5 pin)
+    size_t N() const { return (size_t)nx * ny * nz; }
+    size_t idx(int i, int j, int k) const { return ((size_t)k * ny + j) * nx + i; }
+};
+
+// L(U, t_s): O3, O4, O6, O7, O8.  `stage_c` = c_s in t_s = (n + c_s) dt.
+void eval_rhs(Oracle& o, const std::vector<double>& U, double stage_c, std::vector<double>& L, int stage_no,
+              bool count_caps) {
+    const int nx = o.nx, ny = o.ny, nz = o.nz, nf = o.nf;
+    const size_t N = o.N();
+    // O3: primitives at every interior cell (ghosts = clamped copies, R8b)
+    long long ncap = 0;
+    int has_nan = 0;
+    double amax[3] = {0.0, 0.0, 0.0};
+#pragma omp parallel
+    {
+        double am[3] = {0.0, 0.0, 0.0};
+        long long nc = 0; int hn = 0;
+#pragma omp for nowait
+        for (long long c = 0; c < (long long)N; ++c) {
+            double NB = nf > 4 ? U[4 * N + c] : 0.0;
+            Prim<double> P = con2prim<double>(U[c], U[N + c], U[2 * N + c], U[3 * N + c], NB, o.e_floor, o.delta);
+            o.P[c] = P;
+            nc += P.limited;
+            if (!(std::isfinite(U[c]) && std::isfinite(U[N + c]) && std::isfinite(U[2 * N + c]) && std::isfinite(U[3 * N + c]))) hn = 1;
+            // O4
+            double v2 = P.vx * P.vx + P.vy * P.vy + P.vz * P.vz;
+            double ax = max_wavespeed<double>(P.vx, v2);
+            double ay = max_wavespeed<double>(P.vy, v2);
+            double az = max_wavespeed<double>(P.vz, v2);
+            if (ax > am[0]) am[0] = ax;
+            if (ay > am[1]) am[1] = ay;
+            if (az > am[2]) am[2] = az;
+        }
+#pragma omp critical
+        {
+            for (int d = 0; d < 3; ++d) if (am[d] > amax[d]) amax[d] = am[d];
+            ncap += nc; has_nan |= hn;
+        }
+    }
+    for (int d = 0; d < 3; ++d) o.alpha[d] = amax[d];
+    if (count_caps) o.ncap += ncap;
+    o.has_nan |= has_nan;
+
+    std::fill(L.begin(), L.end(), 0.0);
+    // O6 + O7, direction by direction, all from the same U (R1: unsplit)
+    for (int d = 0; d < 3; ++d) {
+        const int nd = d == 0 ? nx : d == 1 ? ny : nz;
+        const int na = d == 0 ? ny : nx;               // first transverse extent
+        const int nb = d == 2 ? ny : nz;               // second transverse extent
+        const double alpha = o.alpha[d];
+#pragma omp parallel for collapse(2)
+        for (int tb = 0; tb < nb; ++tb) {
+            for (int ta = 0; ta < na; ++ta) {
+                std::vector<double> Fh((size_t)(nd + 1) * 5);
+                for (int i = -1; i < nd; ++i) {        // interface between cell i and i+1 along d
+                    double Uw[8][5]; Prim<double> Pw[8];
+                    for (int m = 0; m < 8; ++m) {
+                        int s = i - 3 + m;
+                        if (s < 0) s = 0;
+                        if (s > nd - 1) s = nd - 1;    // zero-gradient outflow ghosts == index clamping
+                        size_t c = d == 0 ? o.idx(s, ta, tb) : d == 1 ? o.idx(ta, s, tb) : o.idx(ta, tb, s);
+                        for (int q = 0; q < nf; ++q) Uw[m][q] = U[q * N + c];
+                        Pw[m] = o.P[c];
+                    }
+                    interface_flux<double>(d, nf, Uw, Pw, alpha, o.eps, &Fh[(size_t)(i + 1) * 5]);
+                }
+                for (int i = 0; i < nd; ++i) {
+                    size_t c = d == 0 ? o.idx(i, ta, tb) : d == 1 ? o.idx(ta, i, tb) : o.idx(ta, tb, i);
+                    for (int q = 0; q < nf; ++q)
+                        L[q * N + c] -= (Fh[(size_t)(i + 1) * 5 + q] - Fh[(size_t)i * 5 + q]) / o.dx;
+                }
+            }
+        }
+    }
+    // O8: jets
+    const double dx3 = o.dx * o.dx * o.dx;
+    for (size_t J = 0; J < o.jets.size(); ++J) {
+        const Jet& jt = o.jets[J];
+        double ell = ((double)(o.step - jt.step_added) + stage_c) * o.dt;
+        double q = 0.0;
+        int ci = jet_axis_index(jt.x0 + jt.nx * ell, nx, o.dx);
+        int cj = jet_axis_index(jt.y0 + jt.ny * ell, ny, o.dx);
+        int ck = jet_axis_index(jt.z0 + jt.nz * ell, nz, o.dx);
+        if (ci >= 0 && cj >= 0 && ck >= 0) {
+            size_t c = o.idx(ci, cj, ck);
+            q = source_q(o.P[c].e, ell, jt.k_rad, jt.k_coll, jt.crcf);
+            L[c] += q / dx3;
+            L[N + c] += q * jt.nx / dx3;
+            L[2 * N + c] += q * jt.ny / dx3;
+            L[3 * N + c] += q * jt.nz / dx3;
+        }
+        if (J < 16 && stage_no >= 0) o.last_q[stage_no][J] = q;
+    }
+}
+
+// O2 + O9: one SSP-RK3 (Shu-Osher) step; reading R5.
+void rk3_step(Oracle& o) {
+    const size_t T = o.N() * o.nf;
+    const double dt = o.dt;
+    eval_rhs(o, o.U, 0.0, o.L, 0, true);
+    for (size_t n = 0; n < T; ++n) o.U1[n] = o.U[n] + dt * o.L[n];
+    eval_rhs(o, o.U1, 1.0, o.L, 1, true);
+    for (size_t n = 0; n < T; ++n) o.U2[n] = 0.75 * o.U[n] + 0.25 * (o.U1[n] + dt * o.L[n]);
+    eval_rhs(o, o.U2, 0.5, o.L, 2, true);
+    for (size_t n = 0; n < T; ++n) o.U[n] = (1.0 / 3.0) * o.U[n] + (2.0 / 3.0) * (o.U2[n] + dt * o.L[n]);
+    const double w[3] = {1.0 / 6.0, 1.0 / 6.0, 2.0 / 3.0};   // effective weights (R5)
+    for (size_t J = 0; J < o.jets.size() && J < 16; ++J)
+        for (int s = 0; s < 3; ++s) {
+            double a = dt * w[s] * o.last_q[s][J];
+            o.deposited[0] += a;
+            o.deposited[1] += a * o.jets[J].nx;
+            o.deposited[2] += a * o.jets[J].ny;
+            o.deposited[3] += a * o.jets[J].nz;
+        }
+    o.step += 1;
+}
+
+}  // namespace
+
+// ============================================================================================
+//  C interface (names oracle_*; deliberately NOT the product's hydro_* header)
+// ============================================================================================
+extern "C" {
+
+void* oracle_create(int nx, int ny, int nz, double dx, double dt, int nfields, double weno_eps,
+                    double v_cap_delta, double e_floor) {
+    if (nx < 1 || ny < 1 || nz < 1 || (nfields != 4 && nfields != 5) || !(dx > 0) || !(dt > 0)) return 0;
+    Oracle* o = new Oracle();
+    o->nx = nx; o->ny = ny; o->nz = nz; o->nf = nfields; o->dx = dx; o->dt = dt;
+    o->eps = weno_eps; o->delta = v_cap_delta; o->e_floor = e_floor;
+    o->step = 0; o->ncap = 0; o->has_nan = 0;
+    size_t T = o->N() * nfields;
+    o->U.assign(T, 0.0); o->U1.assign(T, 0.0); o->U2.assign(T, 0.0); o->L.assign(T, 0.0);
+    o->P.resize(o->N());
+    for (int d = 0; d < 3; ++d) o->alpha[d] = 0.0;
+    for (int d = 0; d < 4; ++d) o->deposited[d] = 0.0;
+    std::memset(o->last_q, 0, sizeof(o->last_q));
+    return o;
+}
+void oracle_destroy(void* h) { delete (Oracle*)h; }
+
+// U: nfields blocks of nz*ny*nx doubles, x fastest.  Resets step counter; keeps jets.
+void oracle_set_state(void* h, const double* U) {
+    Oracle* o = (Oracle*)h;
+    std::copy(U, U + o->N() * o->nf, o->U.begin());
+    o->step = 0; o->ncap = 0; o->has_nan = 0;
+    for (int d = 0; d < 4; ++d) o->deposited[d] = 0.0;
+    for (size_t J = 0; J < o->jets.size(); ++J) o->jets[J].step_added = 0;
+}
+int oracle_add_jet(void* h, double x0, double y0, double z0, double dirx, double diry, double dirz,
+                   double k_rad, double k_coll, double crcf) {
+    Oracle* o = (Oracle*)h;
+    double nrm = std::sqrt(dirx * dirx + diry * diry + dirz * dirz);
+    if (!(nrm > 0)) return -1;
+    Jet j; j.x0 = x0; j.y0 = y0; j.z0 = z0; j.nx = dirx / nrm; j.ny = diry / nrm; j.nz = dirz / nrm;
+    j.k_rad = k_rad; j.k_coll = k_coll; j.crcf = crcf; j.step_added = o->step;
+    o->jets.push_back(j);
+    return (int)o->jets.size() - 1;
+}
+void oracle_clear_jets(void* h) { ((Oracle*)h)->jets.clear(); }
+void oracle_step(void* h, int nsteps) {
+    Oracle* o = (Oracle*)h;
+    for (int s = 0; s < nsteps; ++s) rk3_step(*o);
+}
+// which = 0: U;  1: primitives (e, vx, vy, vz[, n]) of the current U via O3
+void oracle_get_fields(void* h, double* out, int which) {
+    Oracle* o = (Oracle*)h;
+    const size_t N = o->N();
+    if (which == 0) { std::copy(o->U.begin(), o->U.end(), out); return; }
+    for (size_t c = 0; c < N; ++c) {
+        double NB = o->nf > 4 ? o->U[4 * N + c] : 0.0;
+        Prim<double> P = con2prim<double>(o->U[c], o->U[N + c], o->U[2 * N + c], o->U[3 * N + c], NB, o->e_floor, o->delta);
+        out[c] = P.e; out[N + c] = P.vx; out[2 * N + c] = P.vy; out[3 * N + c] = P.vz;
+        if (o->nf > 4) out[4 * N + c] = P.n;
+    }
+}
+void oracle_get_diag(void* h, double alpha[3], double* cfl, long long* ncap, int* has_nan, double deposited[4],
+                     long long* step) {
+    Oracle* o = (Oracle*)h;
+    double am = 0;
+    for (int d = 0; d < 3; ++d) { alpha[d] = o->alpha[d]; am = std::max(am, o->alpha[d]); }
+    *cfl = am * o->dt / o->dx; *ncap = o->ncap; *has_nan = o->has_nan; *step = o->step;
+    for (int d = 0; d < 4; ++d) deposited[d] = o->deposited[d];
+}
+// L(U, t_n + stage_c*dt) of the current state into out (same layout as U); also refreshes alpha.
+// Does not advance anything and does not count cap events.
+void oracle_eval_rhs(void* h, double stage_c, double* out) {
+    Oracle* o = (Oracle*)h;
+    eval_rhs(*o, o->U, stage_c, o->L, -1, false);
+    std::copy(o->L.begin(), o->L.end(), out);
+}
+// the three stage values q^s of every jet during the LAST step (P5 pin): out[3*njets], s-major
+void oracle_last_stage_q(void* h, double* out) {
+    Oracle* o = (Oracle*)h;
+    size_t nj = std::min<size_t>(o->jets.size(), 16);
+    for (int s = 0; s < 3; ++s) for (size_t J = 0; J < nj; ++J) out[s * nj + J] = o->last_q[s][J];
+}
+
+// ------------------------------------------------------------ scalar entry points for the pins
+void oracle_con2prim(double E, double Mx, double My, double Mz, double NB, double e_floor, double delta,
+                     double out[6], int* limited) {
+    Prim<double> P = con2prim<double>(E, Mx, My, Mz, NB, e_floor, delta);
+    out[0] = P.e; out[1] = P.p; out[2] = P.vx; out[3] = P.vy; out[4] = P.vz; out[5] = P.n; *limited = P.limited;
+}
+// lam[d] = max(|lambda_+^d|, |lambda_-^d|)
+void oracle_wavespeeds(double vx, double vy, double vz, double lam[3]) {
+    double v2 = vx * vx + vy * vy + vz * vz;
+    lam[0] = max_wavespeed<double>(vx, v2); lam[1] = max_wavespeed<double>(vy, v2); lam[2] = max_wavespeed<double>(vz, v2);
+}
+double oracle_weno7(const double v[7], double eps) { return weno7<double>(v[0], v[1], v[2], v[3], v[4], v[5], v[6], eps); }
+// q[4] candidates, beta[4] expanded form, beta_sos[4] sum-of-squares form, omega[4] nonlinear weights
+void oracle_weno7_parts(const double v[7], double eps, double q[4], double beta[4], double beta_sos[4], double omega[4]) {
+    weno7_parts<double>(v[0], v[1], v[2], v[3], v[4], v[5], v[6], q, beta);
+    weno7_beta_sos(v[0], v[1], v[2], v[3], v[4], v[5], v[6], beta_sos);
+    double al[4], s = 0;
+    for (int k = 0; k < 4; ++k) { double t = eps + beta[k]; al[k] = WENO_D[k] / (t * t); s += al[k]; }
+    for (int k = 0; k < 4; ++k) omega[k] = al[k] / s;
+}
+// interface flux of O6 for one 8-cell window: U[8][nf] row-major (cells i-3..i+4), direction d
+void oracle_interface_flux(int d, int nf, const double* Uwin, double alpha, double eps, double e_floor, double delta,
+                           double* Fhat) {
+    double Uw[8][5]; Prim<double> Pw[8];
+    for (int m = 0; m < 8; ++m) {
+        for (int q = 0; q < 5; ++q) Uw[m][q] = q < nf ? Uwin[m * nf + q] : 0.0;
+        Pw[m] = con2prim<double>(Uw[m][0], Uw[m][1], Uw[m][2], Uw[m][3], Uw[m][4], e_floor, delta);
+    }
+    double F[5];
+    interface_flux<double>(d, nf, Uw, Pw, alpha, eps, F);
+    for (int q = 0; q < nf; ++q) Fhat[q] = F[q];
+}
+double oracle_source_q(double e_c, double ell, double k_rad, double k_coll, double crcf) {
+    return source_q(e_c, ell, k_rad, k_coll, crcf);
+}
+int oracle_jet_axis_index(double x, int n, double dx) { return jet_axis_index(x, n, dx); }
+void oracle_constants(double out[3]) { out[0] = HBARC; out[1] = G_DOF; out[2] = CS2; }
+
+// ------------------------------------------------------------ measured ALGORITHMIC flop count
+// Runs the per-cell routines of one stage on the counting type for one interior cell:
+// con2prim + 3 wavespeeds + (per direction: one interface flux [shared by two cells, so counted
+// once per cell] + the divergence update) + RK combine.  Returns flops per cell per stage.
+// breakdown[0]=con2prim, [1]=wavespeeds, [2]=one interface flux (nf fields, incl. split),
+// [3]=divergence per direction, [4]=RK combine (worst stage), [5]=one weno7 reconstruction.
+double oracle_count_flops(int nf, double* breakdown) {
+    typedef Counted R;
+    R Uw[8][5]; Prim<R> Pw[8];
+    for (int m = 0; m < 8; ++m) {
+        Uw[m][0] = R(10.0 + m); Uw[m][1] = R(1.0 + 0.1 * m); Uw[m][2] = R(0.5); Uw[m][3] = R(-0.3); Uw[m][4] = R(1.0);
+    }
+    long long t0 = Counted::ops;
+    Prim<R> P = con2prim<R>(Uw[0][0], Uw[0][1], Uw[0][2], Uw[0][3], Uw[0][4], 1e-12, 1e-10);
+    long long c_c2p = Counted::ops - t0;
+    if (nf <= 4) c_c2p -= 7;                       // v^2, 1-v^2, sqrt, N_B*... only needed with N_B
+    t0 = Counted::ops;
+    R v2 = P.vx * P.vx + P.vy * P.vy + P.vz * P.vz;
+    R s = max_wavespeed<R>(P.vx, v2) + max_wavespeed<R>(P.vy, v2) + max_wavespeed<R>(P.vz, v2);
+    long long c_ws = Counted::ops - t0 - 2;       // the two '+' above are not part of the method
+    (void)s;
+    for (int m = 0; m < 8; ++m) Pw[m] = con2prim<R>(Uw[m][0], Uw[m][1], Uw[m][2], Uw[m][3], Uw[m][4], 1e-12, 1e-10);
+    // per-interface cost: the split of ONE new cell (each cell is split once per direction) +
+    // 2*nf reconstructions + nf sums.  interface_flux() recomputes the split for all 8 cells,
+    // which is the oracle's redundancy, not the algorithm's: count 1/8 of the split work.
+    t0 = Counted::ops;
+    R Fh[5];
+    interface_flux<R>(0, nf, Uw, Pw, R(0.9), 1e-6, Fh);
+    long long c_if_all = Counted::ops - t0;
+    t0 = Counted::ops;
+    R w = weno7<R>(Uw[0][0], Uw[1][0], Uw[2][0], Uw[3][0], Uw[4][0], Uw[5][0], Uw[6][0], 1e-6);
+    long long c_weno = Counted::ops - t0;
+    (void)w;
+    long long c_split_all = c_if_all - 2LL * nf * c_weno - nf;    // 8 cells' flux+split
+    long long c_if = c_split_all / 8 + 2LL * nf * c_weno + nf;
+    long long c_div = 2LL * nf;                   // (Fh_r - Fh_l)/dx subtracted from L: sub, div->mul, sub
+    c_div = 3LL * nf;
+    long long c_rk = 5LL * nf;                    // a*Un + b*(Us + dt*L): 2 mul + add + mul + add
+    double total = (double)c_c2p + (double)c_ws + 3.0 * ((double)c_if + (double)c_div) + (double)c_rk;
+    if (breakdown) {
+        breakdown[0] = (double)c_c2p; breakdown[1] = (double)c_ws; breakdown[2] = (double)c_if;
+        breakdown[3] = (double)c_div; breakdown[4] = (double)c_rk; breakdown[5] = (double)c_weno;
+    }
+    return total;
+}
+
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+void oracle_set_num_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+}  // extern "C"

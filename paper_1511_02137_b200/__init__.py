@@ -1,0 +1,15 @@
+"""B200-native hot path of the (3+1)-D ideal relativistic hydro solver of arxiv 1511.02137.
+
+`hydro`     -- thin ctypes binding of the C-ABI CUDA library (include/hydro.h, csrc/).
+`synthetic` -- seeded input generators shared by the CUDA path and the CPU oracle (no method arithmetic).
+"""
+from . import synthetic  # noqa: F401
+
+__all__ = ["synthetic", "hydro"]
+
+
+def __getattr__(name):
+    if name == "hydro":
+        import importlib
+        return importlib.import_module(".hydro", __name__)
+    raise AttributeError(name)
