@@ -1,0 +1,123 @@
+/* hydro.h -- C ABI of the B200-native hot path of the (3+1)-D ideal relativistic hydrodynamics solver of
+ * arxiv 1511.02137 (Marcinkowski et al.).  One handle = one GPU, one CUDA stream, one Cartesian grid.
+ *
+ * What the library computes (citations are PAPER.md lines):
+ *   d_mu T^{mu nu} = S^nu,  T^{mu nu} = (e+p) u^mu u^nu - p g^{mu nu}           eq. (1)  :17-19
+ *   S^nu = sum_jets (-dE/dt, -dM/dt) delta^3(x - x_jet(t))                        eq. (2)  :21-23
+ *   -dE/dx = kappa_rad (C_R/C_F) T^3 x + kappa_coll (C_R/C_F) T^2                 eq. (3)  :27-31
+ *   7th-order WENO in space, 3rd-order Runge-Kutta in time                        :25
+ *   Cartesian grid, EOS p = e/3, dx = 0.1 fm, dt = 0.02 fm/c, 256^3               :13, :49
+ * for the conserved densities U = (T^00, T^0x, T^0y, T^0z [, N_B]).  Everything the paper leaves open
+ * (Lax-Friedrichs splitting, WENO-JS weights, Shu-Osher RK3, outflow ghosts, delta-function deposit, T(e),
+ * admissibility cap) follows the readings R1-R14 listed in DESIGN.md.
+ *
+ * Conventions
+ *   - every function returns an int status (HYDRO_OK = 0); nothing throws or aborts;
+ *   - pointers are plain host or device pointers as stated per argument (`memspace`); the library never
+ *     keeps or frees a caller's pointer; the caller owns every buffer it passes;
+ *   - field layout: `nfields` contiguous blocks of nz*ny*nx reals, x fastest:
+ *         idx = ((f*nz + k)*ny + j)*nx + i,   interior cells only (ghost cells are never stored);
+ *     element type is double (precision 64) or float (precision 32) as chosen at create;
+ *   - cell (i,j,k) is centred at ((i + 1/2 - nx/2) dx, (j + 1/2 - ny/2) dx, (k + 1/2 - nz/2) dx)  (R6);
+ *   - units: GeV/fm^3 for energy/momentum densities, fm for lengths, fm/c for times, c = 1;
+ *   - all work is enqueued on the handle's stream; calls on one handle must not race (not thread-safe);
+ *   - there is no CPU fallback: without a CUDA device hydro_create fails with HYDRO_ECUDA.
+ */
+#ifndef HYDRO_H_
+#define HYDRO_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hydro hydro_t; /* opaque; owned by the library */
+
+enum { HYDRO_OK = 0, HYDRO_EINVAL = 1, HYDRO_ENOMEM = 2, HYDRO_ECUDA = 3, HYDRO_ESTATE = 4 };
+enum { HYDRO_EOS_CONFORMAL = 0 };             /* p = e/3; the only EOS */
+enum { HYDRO_MEM_HOST = 0, HYDRO_MEM_DEVICE = 1 };
+enum { HYDRO_FIELDS_CONSERVED = 0, HYDRO_FIELDS_PRIMITIVE = 1 };
+
+/* run options ("eos" argument of hydro_create).  A zero in weno_eps / v_cap_delta / e_floor selects the
+ * default of the chosen precision. */
+typedef struct {
+    int    eos;          /* HYDRO_EOS_CONFORMAL */
+    int    nfields;      /* 4 = (T00, T0x, T0y, T0z); 5 adds the baryon density N_B = n gamma (config 4) */
+    int    precision;    /* 64 (fp64) or 32 (fp32 variant, reading R10) */
+    double weno_eps;     /* epsilon of the WENO-JS weights, default 1e-6 (R3) */
+    double v_cap_delta;  /* |M| <= (1 - delta) E in con2prim, default 1e-10 (fp64) / 1e-5 (fp32) (R9, R10) */
+    double e_floor;      /* E >= e_floor in con2prim, default 1e-12 GeV/fm^3 (R9) */
+} hydro_eos_t;
+
+/* Kernel classes timed by hydro_set_profiling / hydro_get_kernel_times. */
+enum { HYDRO_K_PRIM = 0, HYDRO_K_SWEEP_X = 1, HYDRO_K_SWEEP_Y = 2, HYDRO_K_SWEEP_Z = 3, HYDRO_K_SOURCE = 4,
+       HYDRO_K_COUNT = 5 };
+
+/* Create a solver for an nx*ny*nz grid (each >= 1; a direction with fewer than 8 cells still works through
+ * index clamping), spacing dx > 0 [fm] in all directions, fixed step dt > 0 [fm/c].  `eos` may be NULL
+ * (conformal EOS, 4 fields, fp64, default parameters).  `cuda_stream` is a cudaStream_t passed as a void*
+ * (NULL = the library creates and owns a non-blocking stream).  Allocates 3 state copies, one RHS copy and
+ * two primitive fields on the current CUDA device.  Errors: HYDRO_EINVAL, HYDRO_ENOMEM, HYDRO_ECUDA. */
+int hydro_create(hydro_t **out, int nx, int ny, int nz, double dx, double dt, const hydro_eos_t *eos,
+                 void *cuda_stream);
+void hydro_destroy(hydro_t *h);
+
+/* Copy the conserved state in (layout above; `U` is a host pointer for HYDRO_MEM_HOST, a device pointer for
+ * HYDRO_MEM_DEVICE).  Resets the step counter, the time and the diagnostics to 0; jets are kept and restart
+ * from their initial positions at t = 0.  Asynchronous for device memory, synchronous for host memory. */
+int hydro_set_state(hydro_t *h, const void *U, int memspace);
+
+/* Add a jet (eq. 2, 3): position (x0,y0,z0) [fm] relative to the grid centre at the current simulation time,
+ * direction normalised inside (zero vector -> HYDRO_EINVAL), speed c, never deflected or stopped
+ * (PAPER.md:31).  kappa_rad, kappa_coll, cr_over_cf are the coefficients of eq. (3) (paper: 4, 2.5, 1).
+ * `id` (may be NULL) receives the jet index. */
+int hydro_add_jet(hydro_t *h, double x0, double y0, double z0, double dirx, double diry, double dirz,
+                  double kappa_rad, double kappa_coll, double cr_over_cf, int *id);
+int hydro_clear_jets(hydro_t *h);
+
+/* Advance nsteps >= 0 full SSP-RK3 steps of size dt: per stage con2prim + wavespeed max (a-1, a-2), the three
+ * WENO7 Lax-Friedrichs sweeps (a-3, a-4), the jet source (a-5) and the stage combination (a-6), with
+ * zero-gradient outflow ghosts (a-7).  Asynchronous on the handle's stream. */
+int hydro_step(hydro_t *h, int nsteps);
+
+/* Block until everything enqueued on the handle's stream has finished. */
+int hydro_synchronize(hydro_t *h);
+
+/* which = HYDRO_FIELDS_CONSERVED: U (same layout as set_state); HYDRO_FIELDS_PRIMITIVE: (e, vx, vy, vz[, n])
+ * from con2prim of the current state.  `out` holds nfields*nz*ny*nx reals in `memspace`.  Synchronises. */
+int hydro_get_fields(hydro_t *h, void *out, int which, int memspace);
+
+/* L(U, t_n + stage_c*dt) = -sum_d D_d(U) + S of the CURRENT state, written to `out` (layout of U, `memspace`).
+ * Does not advance anything; refreshes alpha.  For stage-level parity tests.  Synchronises. */
+int hydro_eval_rhs(hydro_t *h, double stage_c, void *out, int memspace);
+
+/* Diagnostics (any pointer may be NULL): alpha[3] = Lax-Friedrichs speeds of the last evaluated stage,
+ * cfl = max(alpha) dt/dx, ncap = cumulative number of (cell, stage) events where the con2prim floor/cap fired,
+ * has_nan = a non-finite conserved value was seen, deposited[4] = total (E, Mx, My, Mz) [GeV] added by jets,
+ * step = number of completed steps.  Synchronises. */
+int hydro_get_diag(hydro_t *h, double alpha[3], double *cfl, long long *ncap, int *has_nan, double deposited[4],
+                   long long *step);
+/* q^s [GeV/fm] of jet `jet` in the three stages of the last step (out[3]).  Synchronises. */
+int hydro_get_last_stage_q(hydro_t *h, int jet, double out[3]);
+
+/* Per-kernel-class device times: when enabled, CUDA events bracket every kernel launch of hydro_step on the
+ * handle's stream; hydro_get_kernel_times synchronises and returns accumulated milliseconds and launch counts
+ * per class (arrays of HYDRO_K_COUNT) since profiling was last enabled. */
+int hydro_set_profiling(hydro_t *h, int enable);
+int hydro_get_kernel_times(hydro_t *h, double ms[HYDRO_K_COUNT], long long launches[HYDRO_K_COUNT]);
+
+/* Number of kernel launches hydro_step has enqueued on this handle since create. */
+long long hydro_launch_count(const hydro_t *h);
+
+/* Register-resident DFMA (precision 64) or FFMA (32) chain on every SM of the current device for about
+ * `millis` ms on `cuda_stream`; returns the achieved TFLOP/s (FMA = 2 flops).  The measured ALU peak the
+ * roofline fraction is quoted against. */
+int hydro_measure_alu_peak(int precision, double millis, void *cuda_stream, double *tflops);
+
+const char *hydro_strerror(int code);
+/* Text of the last CUDA error seen by this handle ("" if none). */
+const char *hydro_last_cuda_error(const hydro_t *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HYDRO_H_ */

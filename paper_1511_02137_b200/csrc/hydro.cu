@@ -1,0 +1,479 @@
+// hydro.cu -- C-ABI entry points of include/hydro.h: handle, buffers, launch sequence.  PRODUCT (sm_100a).
+// No CPU fallback: every step of the path runs in the kernels of hydro_kernels.cuh.
+#include "../../include/hydro.h"
+#include "hydro_kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace hydro_dev;
+
+struct hydro {
+    int nx, ny, nz, nf, prec;
+    long long N;
+    double dx, dt, weno_eps, delta, e_floor;
+    size_t esz;                         // bytes per real
+    cudaStream_t stream;
+    bool own_stream;
+    void* buf[3];                       // state copies: buf[cur] = U^n, the other two are stage states
+    int cur;
+    void* L;                            // right-hand side
+    void* P;                            // pressure of the state the primitives were last computed for
+    void* W;                            // scale/(E+p) of that state
+    void* scratch;                      // nf*N reals for get_fields(primitive) / eval_rhs staging
+    Diag* diag;
+    JetDev* jets_dev;
+    std::vector<JetDev> jets;
+    bool jets_dirty;
+    long long step;
+    int prim_slot;                      // DiagSlot holding alpha of buf[cur]'s primitives
+    bool prims_valid;
+    int nseg[3];
+    int num_sms;
+    long long launches;
+    // profiling
+    bool profiling;
+    std::vector<std::pair<int, std::pair<cudaEvent_t, cudaEvent_t> > > ev_inflight;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t> > ev_pool;
+    double k_ms[HYDRO_K_COUNT];
+    long long k_n[HYDRO_K_COUNT];
+    std::string cuda_err;
+};
+
+namespace {
+
+int cuda_fail(hydro* h, cudaError_t e, const char* where) {
+    if (h) {
+        char b[256];
+        snprintf(b, sizeof b, "%s: %s", where, cudaGetErrorString(e));
+        h->cuda_err = b;
+    }
+    return e == cudaErrorMemoryAllocation ? HYDRO_ENOMEM : HYDRO_ECUDA;
+}
+#define CK(call)                                                        \
+    do {                                                                \
+        cudaError_t e_ = (call);                                        \
+        if (e_ != cudaSuccess) return cuda_fail(h, e_, #call);          \
+    } while (0)
+
+struct Timer {                          // brackets one launch with events when profiling is on
+    hydro* h;
+    int cls;
+    cudaEvent_t a, b;
+    bool on;
+    Timer(hydro* h_, int cls_) : h(h_), cls(cls_), a(0), b(0), on(h_->profiling) {
+        if (!on) return;
+        if (!h->ev_pool.empty()) { a = h->ev_pool.back().first; b = h->ev_pool.back().second; h->ev_pool.pop_back(); }
+        else { cudaEventCreate(&a); cudaEventCreate(&b); }
+        cudaEventRecord(a, h->stream);
+    }
+    ~Timer() {
+        if (!on) return;
+        cudaEventRecord(b, h->stream);
+        h->ev_inflight.push_back(std::make_pair(cls, std::make_pair(a, b)));
+    }
+};
+
+void drain_events(hydro* h) {
+    for (size_t n = 0; n < h->ev_inflight.size(); ++n) {
+        float ms = 0.f;
+        cudaEventSynchronize(h->ev_inflight[n].second.second);
+        cudaEventElapsedTime(&ms, h->ev_inflight[n].second.first, h->ev_inflight[n].second.second);
+        h->k_ms[h->ev_inflight[n].first] += ms;
+        h->k_n[h->ev_inflight[n].first] += 1;
+        h->ev_pool.push_back(h->ev_inflight[n].second);
+    }
+    h->ev_inflight.clear();
+}
+
+template <typename R>
+int launch_prim(hydro* h, const void* U, int slot) {
+    CK(cudaMemsetAsync(&h->diag->slot[slot], 0, sizeof(DiagSlot), h->stream));
+    PrimArgs<R> a;
+    a.U = (const R*)U; a.P = (R*)h->P; a.W = (R*)h->W; a.diag = h->diag; a.slot = slot; a.N = h->N;
+    a.e_floor = (R)h->e_floor; a.one_minus_delta = (R)(1.0 - h->delta);
+    long long blocks = (h->N + 255) / 256;
+    long long cap = (long long)h->num_sms * 8;
+    if (blocks > cap) blocks = cap;
+    {
+        Timer t(h, HYDRO_K_PRIM);
+        k_prim<R><<<(unsigned)blocks, 256, 0, h->stream>>>(a);
+    }
+    h->launches += 1;
+    CK(cudaGetLastError());
+    return HYDRO_OK;
+}
+
+template <typename R, int DIR, int MODE>
+int launch_sweep(hydro* h, SweepArgs<R> a) {
+    const int nd = DIR == 0 ? h->nx : DIR == 1 ? h->ny : h->nz;
+    const long long ntrans = h->N / nd;
+    a.nseg = h->nseg[DIR];
+    dim3 grid((unsigned)((ntrans + 127) / 128), (unsigned)h->nf, (unsigned)a.nseg);
+    {
+        Timer t(h, HYDRO_K_SWEEP_X + DIR);
+        k_sweep<R, DIR, MODE><<<grid, 128, 0, h->stream>>>(a);
+    }
+    h->launches += 1;
+    CK(cudaGetLastError());
+    return HYDRO_OK;
+}
+
+template <typename R>
+int upload_jets(hydro* h) {
+    if (!h->jets_dirty) return HYDRO_OK;
+    if (!h->jets.empty())
+        CK(cudaMemcpyAsync(h->jets_dev, h->jets.data(), h->jets.size() * sizeof(JetDev), cudaMemcpyHostToDevice,
+                           h->stream));
+    // the host vector may change before the copy runs: pageable copies are staged synchronously by the runtime
+    h->jets_dirty = false;
+    return HYDRO_OK;
+}
+
+// L(U_in, t_n + stage_c dt) into h->L; if Uout != 0 the last sweep also forms the next stage state.
+template <typename R>
+int eval_stage(hydro* h, const void* Uin, int slot, int stage, double stage_c, bool commit, double rk_weight,
+               void* Uout, const void* Un, double rk_a, double rk_b) {
+    SweepArgs<R> a;
+    a.U = (const R*)Uin; a.P = (const R*)h->P; a.W = (const R*)h->W; a.L = (R*)h->L;
+    a.Un = (const R*)Un; a.Uout = (R*)Uout; a.diag = h->diag; a.slot = slot;
+    a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.nf = h->nf; a.nseg = 1; a.use_un = Un != 0;
+    a.N = h->N;
+    a.eps_eff = (R)(144.0 * h->weno_eps);
+    a.half_inv_dx = (R)(0.5 / h->dx);
+    a.dt = (R)h->dt; a.rk_a = (R)rk_a; a.rk_b = (R)rk_b;
+    int rc;
+    if ((rc = launch_sweep<R, 0, 0>(h, a)) != HYDRO_OK) return rc;
+    if ((rc = launch_sweep<R, 1, 1>(h, a)) != HYDRO_OK) return rc;
+    if ((rc = upload_jets<R>(h)) != HYDRO_OK) return rc;
+    SourceArgs s;
+    s.diag = h->diag; s.jets = h->jets_dev; s.njets = (int)h->jets.size(); s.slot = slot; s.stage = stage;
+    s.commit = commit ? 1 : 0; s.nx = h->nx; s.ny = h->ny; s.nz = h->nz; s.N = h->N; s.step = h->step;
+    s.stage_c = stage_c; s.dx = h->dx; s.dt = h->dt; s.rk_weight = rk_weight;
+    {
+        Timer t(h, HYDRO_K_SOURCE);
+        k_source<R><<<1, 32, 0, h->stream>>>(s, (const R*)h->P, (R*)h->L);
+    }
+    h->launches += 1;
+    CK(cudaGetLastError());
+    if (Uout) rc = launch_sweep<R, 2, 2>(h, a);
+    else rc = launch_sweep<R, 2, 1>(h, a);
+    return rc;
+}
+
+template <typename R>
+int ensure_prims(hydro* h) {
+    if (h->prims_valid) return HYDRO_OK;
+    int rc = launch_prim<R>(h, h->buf[h->cur], h->prim_slot);
+    if (rc == HYDRO_OK) h->prims_valid = true;
+    return rc;
+}
+
+template <typename R>
+int step_impl(hydro* h, int nsteps) {
+    int rc;
+    for (int n = 0; n < nsteps; ++n) {
+        if ((rc = ensure_prims<R>(h)) != HYDRO_OK) return rc;
+        void* Un = h->buf[h->cur];
+        void* Ua = h->buf[(h->cur + 1) % 3];
+        void* Ub = h->buf[(h->cur + 2) % 3];
+        int slot = h->prim_slot;
+        // stage 1: U1 = Un + dt L(Un, t_n)
+        if ((rc = eval_stage<R>(h, Un, slot, 0, 0.0, true, 1.0 / 6.0, Ua, 0, 0.0, 1.0)) != HYDRO_OK) return rc;
+        if ((rc = launch_prim<R>(h, Ua, slot ^ 1)) != HYDRO_OK) return rc;
+        // stage 2: U2 = 3/4 Un + 1/4 (U1 + dt L(U1, t_n + dt))
+        if ((rc = eval_stage<R>(h, Ua, slot ^ 1, 1, 1.0, true, 1.0 / 6.0, Ub, Un, 0.75, 0.25)) != HYDRO_OK) return rc;
+        if ((rc = launch_prim<R>(h, Ub, slot)) != HYDRO_OK) return rc;
+        // stage 3: U^{n+1} = 1/3 Un + 2/3 (U2 + dt L(U2, t_n + dt/2)), written over Un (each cell reads only its own Un)
+        if ((rc = eval_stage<R>(h, Ub, slot, 2, 0.5, true, 2.0 / 3.0, Un, Un, 1.0 / 3.0, 2.0 / 3.0)) != HYDRO_OK)
+            return rc;
+        h->step += 1;
+        if ((rc = launch_prim<R>(h, Un, slot ^ 1)) != HYDRO_OK) return rc;
+        h->prim_slot = slot ^ 1;
+    }
+    return HYDRO_OK;
+}
+
+template <typename R>
+int eval_rhs_impl(hydro* h, double stage_c) {
+    int rc;
+    if ((rc = ensure_prims<R>(h)) != HYDRO_OK) return rc;
+    return eval_stage<R>(h, h->buf[h->cur], h->prim_slot, 0, stage_c, false, 0.0, 0, 0, 0.0, 0.0);
+}
+
+template <typename R>
+int prims_out_impl(hydro* h, void* out) {
+    long long blocks = (h->N + 255) / 256;
+    long long cap = (long long)h->num_sms * 8;
+    if (blocks > cap) blocks = cap;
+    k_prims_out<R><<<(unsigned)blocks, 256, 0, h->stream>>>((const R*)h->buf[h->cur], (R*)out, h->N, h->nf,
+                                                            (R)h->e_floor, (R)(1.0 - h->delta));
+    CK(cudaGetLastError());
+    return HYDRO_OK;
+}
+
+int copy_out(hydro* h, const void* dev_src, void* out, int memspace) {
+    const size_t bytes = (size_t)h->N * h->nf * h->esz;
+    CK(cudaMemcpyAsync(out, dev_src, bytes, memspace == HYDRO_MEM_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice,
+                       h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return HYDRO_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int hydro_create(hydro_t** out, int nx, int ny, int nz, double dx, double dt, const hydro_eos_t* eos, void* cuda_stream) {
+    if (!out) return HYDRO_EINVAL;
+    *out = 0;
+    hydro_eos_t o;
+    o.eos = HYDRO_EOS_CONFORMAL; o.nfields = 4; o.precision = 64; o.weno_eps = 0; o.v_cap_delta = 0; o.e_floor = 0;
+    if (eos) o = *eos;
+    if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0) || !(dt > 0) || !std::isfinite(dx) || !std::isfinite(dt)) return HYDRO_EINVAL;
+    if (o.eos != HYDRO_EOS_CONFORMAL || (o.nfields != 4 && o.nfields != 5) || (o.precision != 64 && o.precision != 32))
+        return HYDRO_EINVAL;
+    if (o.weno_eps < 0 || o.v_cap_delta < 0 || o.v_cap_delta >= 1 || o.e_floor < 0) return HYDRO_EINVAL;
+    if ((long long)nx * ny * nz > (1LL << 40)) return HYDRO_EINVAL;
+    hydro* h = new (std::nothrow) hydro();
+    if (!h) return HYDRO_ENOMEM;
+    h->nx = nx; h->ny = ny; h->nz = nz; h->nf = o.nfields; h->prec = o.precision;
+    h->N = (long long)nx * ny * nz;
+    h->dx = dx; h->dt = dt;
+    h->weno_eps = o.weno_eps > 0 ? o.weno_eps : 1e-6;
+    h->delta = o.v_cap_delta > 0 ? o.v_cap_delta : (o.precision == 64 ? 1e-10 : 1e-5);
+    h->e_floor = o.e_floor > 0 ? o.e_floor : 1e-12;
+    h->esz = o.precision == 64 ? 8 : 4;
+    h->stream = (cudaStream_t)cuda_stream; h->own_stream = false;
+    for (int b = 0; b < 3; ++b) h->buf[b] = 0;
+    h->cur = 0; h->L = h->P = h->W = h->scratch = 0; h->diag = 0; h->jets_dev = 0;
+    h->jets_dirty = false; h->step = 0; h->prim_slot = 0; h->prims_valid = false; h->launches = 0;
+    h->profiling = false;
+    for (int k = 0; k < HYDRO_K_COUNT; ++k) { h->k_ms[k] = 0; h->k_n[k] = 0; }
+    int rc = HYDRO_OK;
+    do {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) { rc = cuda_fail(h, e, "cudaGetDevice"); break; }
+        e = cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) { rc = cuda_fail(h, e, "cudaDeviceGetAttribute"); break; }
+        if (!cuda_stream) {
+            e = cudaStreamCreateWithFlags(&h->stream, cudaStreamNonBlocking);
+            if (e != cudaSuccess) { rc = cuda_fail(h, e, "cudaStreamCreate"); break; }
+            h->own_stream = true;
+        }
+        const size_t fb = (size_t)h->N * h->nf * h->esz;
+        void** ptrs[] = {&h->buf[0], &h->buf[1], &h->buf[2], &h->L};
+        for (int b = 0; b < 4 && rc == HYDRO_OK; ++b) {
+            e = cudaMalloc(ptrs[b], fb);
+            if (e != cudaSuccess) rc = cuda_fail(h, e, "cudaMalloc(state)");
+        }
+        if (rc != HYDRO_OK) break;
+        if ((e = cudaMalloc(&h->P, (size_t)h->N * h->esz)) != cudaSuccess) { rc = cuda_fail(h, e, "cudaMalloc(P)"); break; }
+        if ((e = cudaMalloc(&h->W, (size_t)h->N * h->esz)) != cudaSuccess) { rc = cuda_fail(h, e, "cudaMalloc(W)"); break; }
+        if ((e = cudaMalloc((void**)&h->diag, sizeof(Diag))) != cudaSuccess) { rc = cuda_fail(h, e, "cudaMalloc(diag)"); break; }
+        if ((e = cudaMalloc((void**)&h->jets_dev, sizeof(JetDev) * MAX_JETS)) != cudaSuccess) { rc = cuda_fail(h, e, "cudaMalloc(jets)"); break; }
+        if ((e = cudaMemsetAsync(h->diag, 0, sizeof(Diag), h->stream)) != cudaSuccess) { rc = cuda_fail(h, e, "cudaMemset(diag)"); break; }
+        // segments along the march axis: enough threads to fill the machine on small grids
+        const int nd[3] = {nx, ny, nz};
+        for (int d = 0; d < 3; ++d) {
+            long long threads = (h->N / nd[d]) * h->nf;
+            int seg = 1;
+            while (threads * seg < (long long)h->num_sms * 1024 && nd[d] / (seg * 2) >= 16) seg *= 2;
+            h->nseg[d] = seg;
+        }
+    } while (0);
+    if (rc != HYDRO_OK) {
+        // keep the error text out of reach of the caller: handle is destroyed
+        hydro_destroy(h);
+        return rc;
+    }
+    *out = h;
+    return HYDRO_OK;
+}
+
+void hydro_destroy(hydro_t* h) {
+    if (!h) return;
+    if (h->stream || !h->own_stream) cudaStreamSynchronize(h->stream);
+    drain_events(h);
+    for (size_t n = 0; n < h->ev_pool.size(); ++n) { cudaEventDestroy(h->ev_pool[n].first); cudaEventDestroy(h->ev_pool[n].second); }
+    for (int b = 0; b < 3; ++b) cudaFree(h->buf[b]);
+    cudaFree(h->L); cudaFree(h->P); cudaFree(h->W); cudaFree(h->scratch); cudaFree(h->diag); cudaFree(h->jets_dev);
+    if (h->own_stream && h->stream) cudaStreamDestroy(h->stream);
+    delete h;
+}
+
+int hydro_set_state(hydro_t* h, const void* U, int memspace) {
+    if (!h || !U || (memspace != HYDRO_MEM_HOST && memspace != HYDRO_MEM_DEVICE)) return HYDRO_EINVAL;
+    const size_t bytes = (size_t)h->N * h->nf * h->esz;
+    CK(cudaMemcpyAsync(h->buf[h->cur], U, bytes, memspace == HYDRO_MEM_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice,
+                       h->stream));
+    CK(cudaMemsetAsync(h->diag, 0, sizeof(Diag), h->stream));
+    if (memspace == HYDRO_MEM_HOST) CK(cudaStreamSynchronize(h->stream));
+    h->step = 0;
+    h->prims_valid = false;
+    h->prim_slot = 0;
+    for (size_t j = 0; j < h->jets.size(); ++j) h->jets[j].step_added = 0;
+    h->jets_dirty = true;
+    return HYDRO_OK;
+}
+
+int hydro_add_jet(hydro_t* h, double x0, double y0, double z0, double dirx, double diry, double dirz, double kappa_rad,
+                  double kappa_coll, double cr_over_cf, int* id) {
+    if (!h) return HYDRO_EINVAL;
+    const double nrm = std::sqrt(dirx * dirx + diry * diry + dirz * dirz);
+    if (!(nrm > 0) || !std::isfinite(nrm) || !std::isfinite(x0 + y0 + z0 + kappa_rad + kappa_coll + cr_over_cf)) return HYDRO_EINVAL;
+    if ((int)h->jets.size() >= MAX_JETS) return HYDRO_ESTATE;
+    JetDev j;
+    j.x0 = x0; j.y0 = y0; j.z0 = z0; j.nx = dirx / nrm; j.ny = diry / nrm; j.nz = dirz / nrm;
+    j.k_rad = kappa_rad; j.k_coll = kappa_coll; j.crcf = cr_over_cf; j.step_added = h->step;
+    h->jets.push_back(j);
+    h->jets_dirty = true;
+    if (id) *id = (int)h->jets.size() - 1;
+    return HYDRO_OK;
+}
+
+int hydro_clear_jets(hydro_t* h) {
+    if (!h) return HYDRO_EINVAL;
+    h->jets.clear();
+    h->jets_dirty = true;
+    return HYDRO_OK;
+}
+
+int hydro_step(hydro_t* h, int nsteps) {
+    if (!h || nsteps < 0) return HYDRO_EINVAL;
+    return h->prec == 64 ? step_impl<double>(h, nsteps) : step_impl<float>(h, nsteps);
+}
+
+int hydro_synchronize(hydro_t* h) {
+    if (!h) return HYDRO_EINVAL;
+    CK(cudaStreamSynchronize(h->stream));
+    return HYDRO_OK;
+}
+
+int hydro_get_fields(hydro_t* h, void* out, int which, int memspace) {
+    if (!h || !out || (memspace != HYDRO_MEM_HOST && memspace != HYDRO_MEM_DEVICE)) return HYDRO_EINVAL;
+    if (which == HYDRO_FIELDS_CONSERVED) return copy_out(h, h->buf[h->cur], out, memspace);
+    if (which != HYDRO_FIELDS_PRIMITIVE) return HYDRO_EINVAL;
+    if (memspace == HYDRO_MEM_DEVICE) {
+        int rc = h->prec == 64 ? prims_out_impl<double>(h, out) : prims_out_impl<float>(h, out);
+        if (rc != HYDRO_OK) return rc;
+        CK(cudaStreamSynchronize(h->stream));
+        return HYDRO_OK;
+    }
+    // host destination: stage through the RHS buffer (free between steps)
+    int rc = h->prec == 64 ? prims_out_impl<double>(h, h->L) : prims_out_impl<float>(h, h->L);
+    if (rc != HYDRO_OK) return rc;
+    return copy_out(h, h->L, out, memspace);
+}
+
+int hydro_eval_rhs(hydro_t* h, double stage_c, void* out, int memspace) {
+    if (!h || !out || (memspace != HYDRO_MEM_HOST && memspace != HYDRO_MEM_DEVICE)) return HYDRO_EINVAL;
+    int rc = h->prec == 64 ? eval_rhs_impl<double>(h, stage_c) : eval_rhs_impl<float>(h, stage_c);
+    if (rc != HYDRO_OK) return rc;
+    return copy_out(h, h->L, out, memspace);
+}
+
+int hydro_get_diag(hydro_t* h, double alpha[3], double* cfl, long long* ncap, int* has_nan, double deposited[4],
+                   long long* step) {
+    if (!h) return HYDRO_EINVAL;
+    Diag d;
+    CK(cudaMemcpyAsync(&d, h->diag, sizeof(Diag), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    double am = 0;
+    for (int k = 0; k < 3; ++k) {
+        if (alpha) alpha[k] = d.alpha_last[k];
+        am = d.alpha_last[k] > am ? d.alpha_last[k] : am;
+    }
+    if (cfl) *cfl = am * h->dt / h->dx;
+    if (ncap) *ncap = (long long)d.ncap_total;
+    if (has_nan) *has_nan = d.nan_total ? 1 : 0;
+    if (deposited) for (int k = 0; k < 4; ++k) deposited[k] = d.deposited[k];
+    if (step) *step = h->step;
+    return HYDRO_OK;
+}
+
+int hydro_get_last_stage_q(hydro_t* h, int jet, double out[3]) {
+    if (!h || !out || jet < 0 || jet >= (int)h->jets.size()) return HYDRO_EINVAL;
+    Diag d;
+    CK(cudaMemcpyAsync(&d, h->diag, sizeof(Diag), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    for (int s = 0; s < 3; ++s) out[s] = d.last_q[s][jet];
+    return HYDRO_OK;
+}
+
+int hydro_set_profiling(hydro_t* h, int enable) {
+    if (!h) return HYDRO_EINVAL;
+    CK(cudaStreamSynchronize(h->stream));
+    drain_events(h);
+    h->profiling = enable != 0;
+    if (enable) for (int k = 0; k < HYDRO_K_COUNT; ++k) { h->k_ms[k] = 0; h->k_n[k] = 0; }
+    return HYDRO_OK;
+}
+
+int hydro_get_kernel_times(hydro_t* h, double ms[HYDRO_K_COUNT], long long launches[HYDRO_K_COUNT]) {
+    if (!h) return HYDRO_EINVAL;
+    CK(cudaStreamSynchronize(h->stream));
+    drain_events(h);
+    for (int k = 0; k < HYDRO_K_COUNT; ++k) {
+        if (ms) ms[k] = h->k_ms[k];
+        if (launches) launches[k] = h->k_n[k];
+    }
+    return HYDRO_OK;
+}
+
+long long hydro_launch_count(const hydro_t* h) { return h ? h->launches : -1; }
+
+int hydro_measure_alu_peak(int precision, double millis, void* cuda_stream, double* tflops) {
+    if (!tflops || (precision != 64 && precision != 32) || !(millis > 0)) return HYDRO_EINVAL;
+    hydro* h = 0;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    void* out = 0;
+    CK(cudaMalloc(&out, 64));
+    cudaEvent_t a, b;
+    cudaEventCreate(&a);
+    cudaEventCreate(&b);
+    const int blocks = sms * 8, threads = 256;
+    int iters = 2000;
+    double best = 0, spent = 0;
+    for (int rep = 0; rep < 64 && spent < millis; ++rep) {
+        cudaEventRecord(a, st);
+        if (precision == 64) k_alu_peak<double><<<blocks, threads, 0, st>>>((double*)out, iters, 0.999999, 1e-7);
+        else k_alu_peak<float><<<blocks, threads, 0, st>>>((float*)out, iters, 0.9999f, 1e-4f);
+        cudaEventRecord(b, st);
+        cudaError_t e = cudaEventSynchronize(b);
+        if (e != cudaSuccess) { cudaFree(out); return HYDRO_ECUDA; }
+        float ms = 0;
+        cudaEventElapsedTime(&ms, a, b);
+        const double fl = 2.0 * 64.0 * (double)iters * (double)blocks * threads;
+        if (rep > 0) { const double tf = fl / (ms * 1e-3) * 1e-12; best = tf > best ? tf : best; spent += ms; }
+        if (ms < 2.0f && iters < 400000) iters *= 4;
+    }
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    cudaFree(out);
+    *tflops = best;
+    return HYDRO_OK;
+}
+
+const char* hydro_strerror(int code) {
+    switch (code) {
+        case HYDRO_OK: return "ok";
+        case HYDRO_EINVAL: return "invalid argument";
+        case HYDRO_ENOMEM: return "out of device memory";
+        case HYDRO_ECUDA: return "CUDA error (see hydro_last_cuda_error)";
+        case HYDRO_ESTATE: return "invalid state (too many jets)";
+        default: return "unknown error";
+    }
+}
+
+const char* hydro_last_cuda_error(const hydro_t* h) { return h ? h->cuda_err.c_str() : ""; }
+
+}  // extern "C"

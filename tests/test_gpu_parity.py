@@ -1,0 +1,292 @@
+"""GPU parity (pin P9): the CUDA path, called through the C ABI, against the CPU oracle on the same seeded inputs.
+
+Error metric (reading R13): err_f = max_cells |f_gpu - f_oracle| / max_cells |f_oracle| per conserved field; a field
+that is identically zero in the oracle must be exactly zero on the GPU.  Tolerance: 1e-9 in fp64 after the run
+(north_star), tighter for single kernels / single stages.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_1511_02137_b200 import synthetic as S
+
+pytestmark = pytest.mark.gpu
+
+TOL_RUN = 1e-9          # north_star: after the run, fp64
+TOL_STAGE = 1e-12       # one evaluation of L(U): only rounding-order differences
+
+
+@pytest.fixture(scope="module")
+def H():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    from paper_1511_02137_b200 import hydro
+    hydro.load()
+    return hydro
+
+
+def r13(gpu, ref):
+    errs = []
+    for f in range(ref.shape[0]):
+        m = np.max(np.abs(ref[f]))
+        if m == 0.0:
+            assert np.all(gpu[f] == 0.0), "field %d must be exactly zero" % f
+            errs.append(0.0)
+        else:
+            errs.append(float(np.max(np.abs(gpu[f] - ref[f])) / m))
+    return errs
+
+
+def make_pair(H, oracle, cfg, noise=True, jets=True, **kw):
+    c = S.CONFIGS[cfg] if not isinstance(cfg, dict) else cfg
+    U0 = S.make_state(c, noise=noise)
+    g = H.Hydro(*c["n"], c["dx"], c["dt"], nfields=c["nf"], **kw)
+    o = oracle.Oracle(*c["n"], c["dx"], c["dt"], nfields=c["nf"])
+    g.set_state(U0)
+    o.set_state(U0)
+    if jets:
+        for pos, d in c["jets"]:
+            g.add_jet(pos, d, S.KAPPA_RAD, S.KAPPA_COLL, S.CR_OVER_CF)
+            o.add_jet(pos, d, S.KAPPA_RAD, S.KAPPA_COLL, S.CR_OVER_CF)
+    return c, U0, g, o
+
+
+def compare_diag(g, o, steps):
+    dg, do = g.diag(), o.diag()
+    assert dg["step"] == do["step"] == steps
+    assert np.max(np.abs(dg["alpha"] - do["alpha"])) < 1e-12
+    assert abs(dg["cfl"] - do["cfl"]) < 1e-12
+    assert dg["has_nan"] == do["has_nan"] == 0
+    assert np.max(np.abs(dg["deposited"] - do["deposited"])) <= 1e-10 * max(1e-300, np.max(np.abs(do["deposited"])))
+    return dg, do
+
+
+# ------------------------------------------------------------------------------------------------ a-1, a-2
+def test_con2prim_parity(H, oracle):
+    rng = np.random.default_rng(42)
+    n = (37, 19, 23)                                     # ragged: not a multiple of any block size
+    N = n[0] * n[1] * n[2]
+    e = 10.0 ** rng.uniform(-3, 3, N)
+    vm = rng.uniform(0, 0.999, N)
+    d = rng.normal(size=(3, N))
+    d /= np.linalg.norm(d, axis=0)
+    u = vm / np.sqrt(1 - vm * vm) * d
+    U = S.prim_to_cons(e, u[0], u[1], u[2], e / 10).reshape(5, n[2], n[1], n[0])
+    # a few inadmissible cells: cap and floor must act identically (R9)
+    U[1, 0, 0, :5] = 2.0 * U[0, 0, 0, :5]
+    U[0, 1, 1, :3] = -1.0
+    for nf in (4, 5):
+        g = H.Hydro(*n, 0.1, 0.02, nfields=nf)
+        o = oracle.Oracle(*n, 0.1, 0.02, nfields=nf)
+        g.set_state(U[:nf].copy())
+        o.set_state(U[:nf].copy())
+        Pg, Po = g.get_fields(H.FIELDS_PRIMITIVE), o.get_fields(1)
+        assert np.array_equal(g.get_fields(H.FIELDS_CONSERVED), U[:nf])          # state round-trips bitwise
+        gam2 = 1.0 / (1.0 - np.minimum(vm, 0.9999) ** 2).reshape(n[2], n[1], n[0])
+        capped = np.zeros(gam2.shape, bool)
+        capped[0, 0, :5] = True
+        capped[1, 1, :3] = True
+        assert np.max((np.abs(Pg[0] - Po[0]) / (np.abs(Po[0]) * gam2))[~capped]) < 5e-15
+        # on the cap e = 3(E^2-M^2)/(E+s) cancels to ~2 delta E: compare relative to E, not to e
+        assert np.max((np.abs(Pg[0] - Po[0]) / np.maximum(np.abs(U[0]), 1e-12))[capped]) < 5e-15
+        for f in (1, 2, 3):
+            assert np.max(np.abs(Pg[f] - Po[f])) < 5e-15
+        if nf == 5:
+            assert np.max((np.abs(Pg[4] - Po[4]) / np.abs(Po[4]))[~capped]) < 1e-12 * gam2.max()
+            # on the cap 1 - v^2 ~ 2 delta is itself only known to ~1e-16/delta
+            assert np.max((np.abs(Pg[4] - Po[4]) / np.abs(Po[4]))[capped]) < 1e-5
+        # wavespeed maxima and cap counts come out of one RHS evaluation
+        g.eval_rhs(0.0)
+        o.eval_rhs(0.0)
+        dg, do = g.diag(), o.diag()
+        assert np.max(np.abs(dg["alpha"] - do["alpha"])) < 1e-13
+        g.close(), o.close()
+
+
+# ------------------------------------------------------------------------------------------------ a-3..a-5, a-7
+@pytest.mark.parametrize("n", [(32, 32, 32), (37, 19, 23), (7, 5, 3), (1, 1, 40), (130, 9, 6)])
+@pytest.mark.parametrize("nf", [4, 5])
+def test_rhs_single_stage_parity(H, oracle, n, nf):
+    c = S.scaled_config(0, n)
+    c["nf"] = nf
+    c["jets"] = [((-0.12, 0.03, 0.0), (1.0, 0.5, -0.25))]
+    c, U0, g, o = make_pair(H, oracle, c)
+    for stage_c in (0.0, 1.0, 0.5):
+        Lg, Lo = g.eval_rhs(stage_c), o.eval_rhs(stage_c)
+        scale = np.max(np.abs(Lo), axis=(1, 2, 3))
+        for f in range(nf):
+            assert np.max(np.abs(Lg[f] - Lo[f])) <= TOL_STAGE * max(scale[f], scale[0]), (f, stage_c)
+        assert np.max(np.abs(g.diag()["alpha"] - o.diag()["alpha"])) < 1e-13
+    g.close(), o.close()
+
+
+def test_jet_cell_and_source_bitwise_location(H, oracle):
+    """The deposit cell is integer work: the set of cells touched by the source must be identical."""
+    c = S.scaled_config(0, (24, 20, 16))
+    c["jets"] = [((0.0, 0.0, 0.0), (1.0, 0.0, 0.0)), ((0.0, 0.0, 0.0), (-1.0, 0.0, 0.0)),
+                 ((-0.35, 0.25, 0.05), (0.3, -0.4, 0.2)), ((9.0, 0.0, 0.0), (1.0, 0.0, 0.0))]
+    for stage_c in (0.0, 0.5, 1.0):
+        _, U0, g, o = make_pair(H, oracle, c)
+        _, _, g0, o0 = make_pair(H, oracle, c, jets=False)
+        dLg = g.eval_rhs(stage_c) - g0.eval_rhs(stage_c)
+        dLo = o.eval_rhs(stage_c) - o0.eval_rhs(stage_c)
+        assert np.array_equal(dLg != 0, dLo != 0)
+        assert np.max(np.abs(dLg - dLo)) < 1e-12 * np.max(np.abs(dLo))
+        for x in (g, o, g0, o0):
+            x.close()
+
+
+# ------------------------------------------------------------------------------------------------ whole path
+def test_config0_full_run(H, oracle):
+    c, U0, g, o = make_pair(H, oracle, 0)
+    g.step(c["steps"])
+    o.step(c["steps"])
+    errs = r13(g.get_fields(), o.get_fields())
+    assert max(errs) < TOL_RUN, errs
+    dg, do = compare_diag(g, o, c["steps"])
+    assert dg["ncap"] == do["ncap"] == 0
+    assert np.max(np.abs(g.last_stage_q() - o.last_stage_q())) < 1e-11
+    assert do["deposited"][0] > 0
+    # split stepping gives the same state as one call (the step counter, jets and primitives carry over)
+    g2 = H.Hydro(*c["n"], c["dx"], c["dt"])
+    g2.set_state(U0)
+    for pos, d in c["jets"]:
+        g2.add_jet(pos, d)
+    for k in (3, 0, 6, 1):
+        g2.step(k)
+    assert np.array_equal(g2.get_fields(), g.get_fields())
+    for x in (g, g2, o):
+        x.close()
+
+
+def test_config0_five_fields_and_ragged_grid(H, oracle):
+    c = S.scaled_config(0, (45, 27, 18))
+    c["nf"] = 5
+    c["steps"] = 6
+    c, U0, g, o = make_pair(H, oracle, c)
+    g.step(c["steps"])
+    o.step(c["steps"])
+    errs = r13(g.get_fields(), o.get_fields())
+    assert max(errs) < TOL_RUN, errs
+    compare_diag(g, o, c["steps"])
+    Pg, Po = g.get_fields(H.FIELDS_PRIMITIVE), o.get_fields(1)
+    assert max(r13(Pg, Po)) < TOL_RUN
+    g.close(), o.close()
+
+
+def test_config1_shock_tube(H, oracle):
+    """BASELINE config 1: 512x8x8, 375 steps; GPU vs oracle, and GPU vs the exact Riemann solution (pin P4)."""
+    from test_oracle_riemann import exact_solution, exact_profile
+    c, U0, g, _o = make_pair(H, oracle, 1)
+    _o.close()
+    g.step(c["steps"])
+    Ug = g.get_fields()
+    Pg = g.get_fields(H.FIELDS_PRIMITIVE)
+    # P7 on the GPU: the embedded tube is independent of j, k bitwise and has no transverse momentum
+    assert np.array_equal(Ug, np.broadcast_to(Ug[:, :1, :1, :], Ug.shape))
+    assert np.all(Ug[2] == 0) and np.all(Ug[3] == 0)
+    # the oracle run of the same tube is 1-D (P7: embedding is bitwise in the oracle too)
+    o = oracle.Oracle(512, 1, 1, c["dx"], c["dt"])
+    o.set_state(U0[:, :1, :1, :].copy())
+    o.step(c["steps"])
+    Uo = o.get_fields()
+    errs = r13(Ug[:, :1, :1, :], Uo)
+    assert max(errs) < TOL_RUN, errs
+    x = S.cell_centres(512, c["dx"])
+    ee, ve = exact_profile(x, c["dt"] * c["steps"], exact_solution())
+    assert np.sum(np.abs(Pg[0, 0, 0] - ee)) * c["dx"] < 0.08
+    assert np.sum(np.abs(Pg[1, 0, 0] - ve)) * c["dx"] < 0.01
+    dg = g.diag()
+    assert dg["ncap"] == 0 and abs(dg["alpha"][0] - o.diag()["alpha"][0]) < 1e-12
+    g.close(), o.close()
+
+
+def test_jet_run_with_cap_events(H, oracle):
+    """A jet through e ~ 30 GeV/fm^3 drives cells next to the deposit inadmissible (R9): the cap must fire on
+    both sides in (nearly) the same cells and parity must survive it."""
+    c = S.scaled_config(2, (64, 32, 32))
+    c["jets"] = [((-2.0, 0.0, 0.0), (1.0, 0.0, 0.0))]
+    steps = int(os.environ.get("HYDRO_TEST_CAP_STEPS", "60"))
+    c, U0, g, o = make_pair(H, oracle, c)
+    g.step(steps)
+    o.step(steps)
+    errs = r13(g.get_fields(), o.get_fields())
+    assert max(errs) < TOL_RUN, errs
+    dg, do = compare_diag(g, o, steps)
+    assert do["ncap"] > 0, "this case is meant to exercise the cap"
+    assert abs(dg["ncap"] - do["ncap"]) <= max(2, 0.02 * do["ncap"])
+    g.close(), o.close()
+
+
+def test_config2_midsize(H, oracle):
+    """BASELINE config 2 (128^3); HYDRO_TEST_CFG2_STEPS (default 4) of its 50 steps -- the oracle costs ~9 s/step
+    on 8 cores."""
+    steps = int(os.environ.get("HYDRO_TEST_CFG2_STEPS", "4"))
+    c, U0, g, o = make_pair(H, oracle, 2)
+    g.step(steps)
+    o.step(steps)
+    errs = r13(g.get_fields(), o.get_fields())
+    assert max(errs) < TOL_RUN, errs
+    compare_diag(g, o, steps)
+    g.close(), o.close()
+
+
+# ------------------------------------------------------------------------------------------------ invariants on the GPU
+def test_gpu_uniform_state_and_symmetry(H):
+    n = (40, 24, 17)
+    ones = np.ones((n[2], n[1], n[0]))
+    U0 = S.prim_to_cons(3.7 * ones, 0.3 * ones, -0.2 * ones, 0.1 * ones)
+    g = H.Hydro(*n, 0.1, 0.02)
+    g.set_state(U0)
+    assert np.all(g.eval_rhs(0.0) == 0.0)               # P2: bitwise
+    g.step(3)
+    U = g.get_fields()
+    assert np.array_equal(U, np.broadcast_to(U[:, :1, :1, :1], U.shape))
+    g.close()
+    n = (32, 24, 20)                                     # P6: mirror symmetry
+    U0 = S.gaussian_flow(n, 0.1, peak=10.0, sigma=(0.5, 0.4, 0.6), R=(1.0, 0.8, 1.2), ucoef=0.2, noise=0.0)
+    g = H.Hydro(*n, 0.1, 0.02)
+    g.set_state(U0)
+    g.step(4)
+    U = g.get_fields()
+    g.close()
+    scale = np.abs(U).max(axis=(1, 2, 3))
+    for axis, odd in ((3, 1), (2, 2), (1, 3)):
+        F = np.flip(U, axis=axis)
+        for f in range(4):
+            sign = -1.0 if f == odd else 1.0
+            assert np.max(np.abs(U[f] - sign * F[f])) <= 1e-13 * scale[f]
+
+
+def test_device_pointers_and_streams(H, oracle):
+    """set_state / get_fields with device memory (torch tensors) on a caller-owned torch stream."""
+    import torch
+    c = S.CONFIGS[0]
+    U0 = S.make_state(0)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        Ud = torch.from_numpy(U0).cuda()
+    st.synchronize()
+    g = H.Hydro(*c["n"], c["dx"], c["dt"], stream=st)
+    g.set_state(Ud)
+    g.step(2)
+    out = torch.empty_like(Ud)
+    g.get_fields(out=out)
+    g2 = H.Hydro(*c["n"], c["dx"], c["dt"])
+    g2.set_state(U0)
+    g2.step(2)
+    assert np.array_equal(out.cpu().numpy(), g2.get_fields())
+    assert g.launch_count() == 2 * (3 * 5) + 1
+    g.close(), g2.close()
+
+
+def test_error_paths(H):
+    g = H.Hydro(8, 8, 8, 0.1, 0.02)
+    with pytest.raises(H.HydroError):
+        g.add_jet((0, 0, 0), (0, 0, 0))
+    with pytest.raises(H.HydroError):
+        g.step(-1)
+    g.close()
+    with pytest.raises(H.HydroError):
+        H.Hydro(8, 8, 8, 0.1, 0.0)
