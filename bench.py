@@ -1,0 +1,300 @@
+#!/usr/bin/env python
+"""bench.py -- cell-updates/s of the hot path (BASELINE.json `metric`) on BASELINE config 3.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--precision 64|32]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+
+A "step" is one full SSP-RK3 step (three stage evaluations of con2prim + wavespeed max, the three WENO7-LF
+sweeps, the jet source and the stage combination) of the synthetic 256^3 ellipsoidal-flow + 1 jet grid
+(config 3: PAPER.md:49 for grid/dx/dt, :37 for the IC family; numbers from BASELINE.json, DESIGN.md "Input
+recipe").  The path is one-GPU (north_star); with N > 1 every rank advances its own replica of the grid
+("replicas only") and the value is the aggregate.
+
+One JSON line on stdout (rank 0).  Keys: the contract of the task statement + `roofline` (dominant kernel
+class = the three sweep kernels, bound "alu": FP64 pipe) + `cpu_baseline` (the oracle, timed on the host cores
+on a bounded slab of the same workload).
+
+`--impl reference`: the oracle (oracle/hydro_oracle.cpp) as it stands on the host cores, each step one RK3
+step of a 256 x 256 x NZ slab of the same initial condition (NZ chosen so the run stays within minutes).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1511_02137_b200 import synthetic as S  # noqa: E402
+
+METRIC = "cell-updates/s (full RK3 steps x cells / s)"
+UNIT = "cell-updates/s"
+# Algorithmic flops per cell per stage evaluation, nf = 4 / 5: measured by running the oracle's per-cell routines
+# on an operation-counting number type (oracle_count_flops): FMA = 2, + - * / sqrt = 1.
+# Of these the sweep kernels carry interface_flux + divergence (+ the stage combination in the last sweep).
+FLOPS_STAGE = {4: 3764.0, 5: 4691.0}
+FLOPS_SWEEPS_STAGE = {4: 3 * (1208.0 + 12.0) + 20.0, 5: 3 * (1510.0 + 15.0) + 25.0}
+FP64_NOMINAL_TF = 148 * 64 * 2 * 1.965e9 / 1e12          # 148 SMs x 64 DFMA/clk x 2 x 1.965 GHz = 37.2
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons of one GPU while the timed region runs (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows = []
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.t = threading.Thread(target=self._read, daemon=True)
+        self.t.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        inside = [r for (t, r) in self.rows if t0 <= t <= t1] or [r for (_, r) in self.rows[-3:]]
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in inside:
+            c = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1])); pw.append(float(c[2]))
+            except (ValueError, IndexError):
+                continue
+            for k, nm in enumerate(names):
+                if len(c) > 3 + k and c[3 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_slab_run(cfg, nzs, steps, warmup=0):
+    """Oracle on the central nzs planes of config `cfg`'s initial condition; returns (cells, seconds, threads)."""
+    from oracle import oracle as O
+    c = S.CONFIGS[cfg]
+    nx, ny, nz = c["n"]
+    k0 = nz // 2 - nzs // 2
+    U0 = S.make_state(cfg, z_range=(k0, k0 + nzs))
+    o = O.Oracle(nx, ny, nzs, c["dx"], c["dt"], nfields=c["nf"])
+    o.set_state(U0)
+    for pos, d in c["jets"]:
+        o.add_jet(pos, d, S.KAPPA_RAD, S.KAPPA_COLL, S.CR_OVER_CF)
+    if warmup:
+        o.step(warmup)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    assert o.diag()["has_nan"] == 0
+    o.close()
+    return nx * ny * nzs, dt, O.num_threads()
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    cfg = args.config
+    c = S.CONFIGS[cfg]
+    # size the slab so that (K + W) steps take about two minutes: calibrate on one step of 8 planes
+    cells8, t8, threads = oracle_slab_run(cfg, 8, 1)
+    budget = 120.0
+    nzs = int(min(c["n"][2], max(8, 8 * int(budget / (t8 * (args.steps + args.warmup)) + 1e-9))))
+    cells, secs, threads = oracle_slab_run(cfg, nzs, args.steps, args.warmup)
+    value = cells * args.steps / secs
+    sample = "%dx%dx%d central slab of config %d's IC + jet, %d RK3 steps" % (c["n"][0], c["n"][1], nzs, cfg,
+                                                                              args.steps)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(args, cfg),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }), flush=True)
+
+
+def workload_config(args, cfg):
+    c = S.CONFIGS[cfg]
+    return {"workload": "BASELINE config %d: %dx%dx%d, dx=%g fm, dt=%g fm/c, nf=%d, p=e/3, ellipsoidal flow + %d jet(s), "
+                        "outflow ghosts" % (cfg, c["n"][0], c["n"][1], c["n"][2], c["dx"], c["dt"], c["nf"],
+                                            len(c["jets"])),
+            "cells": int(np.prod(c["n"])), "config_steps": c["steps"],
+            "parallelism": "replicas x%d" % args.gpus,
+            "l2": "state (%.0f MiB per copy) exceeds L2; no flush needed" %
+                  (np.prod(c["n"]) * c["nf"] * (args.precision // 8) / 2 ** 20)}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=120)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1511_02137_b200 import hydro as H
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    H.load()
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = args.config
+    c = S.CONFIGS[cfg]
+    cells = int(np.prod(c["n"]))
+    tdt = torch.float64 if args.precision == 64 else torch.float32
+    U0 = S.make_state(cfg)
+    U0h = torch.from_numpy(U0).to(tdt).pin_memory()
+    outh = torch.empty_like(U0h).pin_memory()
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        U0d = U0h.cuda(non_blocking=True)
+    stream.synchronize()
+    g = H.Hydro(*c["n"], c["dx"], c["dt"], nfields=c["nf"], precision=args.precision, stream=stream)
+    for pos, d in c["jets"]:
+        g.add_jet(pos, d, S.KAPPA_RAD, S.KAPPA_COLL, S.CR_OVER_CF)
+
+    # ---- measured ALU peak of this GPU, same run
+    peak_tf = H.measure_alu_peak(args.precision, 200.0, stream.cuda_stream)
+
+    # ---- warm-up, then the device-resident timed region: K steps from the initial state
+    g.set_state(U0d)
+    g.step(args.warmup)
+    g.set_state(U0d)
+    g.synchronize()
+    sampler = ClockSampler(local if "CUDA_VISIBLE_DEVICES" not in os.environ else
+                           os.environ["CUDA_VISIBLE_DEVICES"].split(",")[local])
+    sampler.start()
+    time.sleep(0.3)
+    g.set_profiling(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0 = g.launch_count()
+    barrier()
+    w0 = time.perf_counter()
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        g.step(args.steps)
+        e1.record(stream)
+    barrier()
+    w1 = time.perf_counter()
+    ms = e0.elapsed_time(e1)
+    launches = g.launch_count() - n0
+    kt = g.kernel_times()
+    g.set_profiling(False)
+    clocks = sampler.stop(w0, w1)
+    dg = g.diag()
+    if dg["has_nan"]:
+        raise SystemExit("bench.py: non-finite state after the timed run")
+
+    # ---- end to end through the C ABI with HOST buffers: upload, K steps, download, all inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        barrier()
+        t0 = time.perf_counter()
+        g.set_state(U0h)
+        g.step(args.steps)
+        g.get_fields(out=outh)
+        torch.cuda.synchronize()
+        t_e2e = time.perf_counter() - t0
+        nbytes = U0h.numel() * U0h.element_size()
+        e2e = (t_e2e, nbytes)
+
+    tmax = torch.tensor([ms, e2e[0] if e2e else 0.0], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_max, e2e_max = tmax.tolist()
+
+    if rank == 0:
+        value = world * cells * args.steps / (ms_max * 1e-3)
+        nf = c["nf"]
+        sweeps = [kt[k] for k in ("sweep_x", "sweep_y", "sweep_z")]
+        sw_ms = sum(k["ms"] for k in sweeps)
+        sw_n = sum(k["launches"] for k in sweeps)
+        all_ms = sum(k["ms"] for k in kt.values())
+        # dominant kernel class: the WENO7-LF sweep kernels; flops per launch = (sweep flops per cell per stage / 3) * cells
+        fl_launch = FLOPS_SWEEPS_STAGE[nf] / 3.0 * cells
+        achieved = fl_launch / (sw_ms / sw_n * 1e-3) / 1e12 if sw_n else 0.0
+        nominal = FP64_NOMINAL_TF * (1 if args.precision == 64 else 2)
+        roof = {"bound": "alu", "kernel": "k_sweep<x|y|z> (WENO7-LF flux + divergence [+ RK3 combine])",
+                "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf,
+                "peak_kind": "measured in this run: register-resident %s chain on all SMs (hydro_measure_alu_peak)" %
+                             ("DFMA" if args.precision == 64 else "FFMA"),
+                "peak_nominal": nominal, "frac_of_nominal": achieved / nominal,
+                "flops_per_launch": fl_launch, "avg_launch_ms": sw_ms / sw_n if sw_n else None,
+                "share_of_step": sw_ms / all_ms if all_ms else None,
+                "kernel_ms_per_step": {k: v["ms"] / args.steps for k, v in kt.items()},
+                "whole_path_frac": (FLOPS_STAGE[nf] * 3 * value) / (peak_tf * 1e12),
+                "traffic": None}
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.precision == 64 else "f32",
+            "data": "synthetic", "config": workload_config(args, cfg), "clocks": clocks,
+            "gpu_launches": int(launches), "roofline": roof,
+            "diag": {"ncap": dg["ncap"], "alpha": dg["alpha"].tolist(), "deposited_E_GeV": float(dg["deposited"][0])},
+        }
+        if e2e:
+            line["e2e"] = {"value": world * cells * args.steps / e2e_max, "unit": UNIT,
+                           "h2d_bytes_per_step": e2e[1] / args.steps, "d2h_bytes_per_step": e2e[1] / args.steps,
+                           "what": "hydro_set_state(host) + hydro_step(K) + hydro_get_fields(host), pinned buffers; "
+                                   "bytes are the one upload / one download spread over K steps"}
+        if not args.no_cpu_baseline and world == 1:
+            cells_s, secs, threads = oracle_slab_run(cfg, 16, 2)
+            line["cpu_baseline"] = {"value": cells_s * 2 / secs, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                    "sample": "%dx%dx16 central slab of config %d's IC + jet, 2 RK3 steps (%.1f s)" %
+                                              (c["n"][0], c["n"][1], cfg, secs)}
+        print(json.dumps(line), flush=True)
+    g.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

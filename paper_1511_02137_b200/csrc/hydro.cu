@@ -2,9 +2,13 @@
 // No CPU fallback: every step of the path runs in the kernels of hydro_kernels.cuh.
 #include "../../include/hydro.h"
 #include "hydro_kernels.cuh"
+#include "hydro_sweep_tma.cuh"
+
+#include <cudaTypedefs.h>
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -33,6 +37,11 @@ struct hydro {
     int prim_slot;                      // DiagSlot holding alpha of buf[cur]'s primitives
     bool prims_valid;
     int nseg[3];
+    // TMA sweeps (fp64, even nx): tensor maps per state copy and direction, march cells per block
+    bool use_tma;
+    int tma_dirs;                       // bit d: direction d uses the TMA sweep (HYDRO_TMA_DIRS, default 7)
+    CUtensorMap mapU[3][3], mapW[3], mapP[3], mapL;
+    int seg_len[3], tma_nseg[3];
     int num_sms;
     long long launches;
     // profiling
@@ -108,8 +117,110 @@ int launch_prim(hydro* h, const void* U, int slot) {
     return HYDRO_OK;
 }
 
+int buf_index(const hydro* h, const void* U) {
+    for (int b = 0; b < 3; ++b) if (h->buf[b] == U) return b;
+    return -1;
+}
+
+template <int DIR, int MODE, int NF>
+int launch_sweep_tma_nf(hydro* h, const SweepArgs<double>& a0) {
+    SweepArgs<double> a = a0;
+    const int b = buf_index(h, a.U);
+    if (b < 0) return HYDRO_ESTATE;
+    SweepMaps m;
+    m.U = h->mapU[b][DIR]; m.W = h->mapW[DIR]; m.P = h->mapP[DIR]; m.Lst = h->mapL;
+    a.seg_len = h->seg_len[DIR];
+    const int nlane = DIR == 0 ? h->ny : h->nx;
+    const int other = DIR == 2 ? h->ny : h->nz;
+    dim3 grid((unsigned)(((nlane + 31) / 32) * other), (unsigned)h->tma_nseg[DIR], 1);
+    dim3 block(32, NF, 1);
+    const int smem = sweep_tma_smem_bytes(NF, DIR, 8);
+    {
+        Timer t(h, HYDRO_K_SWEEP_X + DIR);
+        k_sweep_tma<DIR, MODE, NF><<<grid, block, smem, h->stream>>>(m, a);
+    }
+    h->launches += 1;
+    CK(cudaGetLastError());
+    return HYDRO_OK;
+}
+
+template <int DIR, int MODE>
+int launch_sweep_tma(hydro* h, const SweepArgs<double>& a) {
+    return h->nf == 4 ? launch_sweep_tma_nf<DIR, MODE, 4>(h, a) : launch_sweep_tma_nf<DIR, MODE, 5>(h, a);
+}
+template <int DIR, int MODE>
+int launch_sweep_tma(hydro*, const SweepArgs<float>&) { return HYDRO_ESTATE; }
+
+template <int DIR, int MODE, int NF>
+int set_smem_attr() {
+    return cudaFuncSetAttribute(k_sweep_tma<DIR, MODE, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                sweep_tma_smem_bytes(NF, DIR, 8)) == cudaSuccess ? 0 : 1;
+}
+
+// 4-D tensor map (x, y, z, field) of one SoA buffer with `nfb` fields; box given per dimension
+int make_map(hydro* h, CUtensorMap* out, void* base, int nfb, const unsigned box[4], bool swizzle64) {
+    static PFN_cuTensorMapEncodeTiled_v12000 encode = 0;
+    if (!encode) {
+        void* fn = 0;
+        cudaDriverEntryPointQueryResult q;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q);
+        if (e != cudaSuccess || q != cudaDriverEntryPointSuccess || !fn) {
+            h->cuda_err = "cuTensorMapEncodeTiled entry point not available";
+            return HYDRO_ECUDA;
+        }
+        encode = (PFN_cuTensorMapEncodeTiled_v12000)fn;
+    }
+    cuuint64_t gdim[4] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny, (cuuint64_t)h->nz, (cuuint64_t)nfb};
+    cuuint64_t gstr[3] = {(cuuint64_t)h->nx * 8, (cuuint64_t)h->nx * h->ny * 8, (cuuint64_t)h->N * 8};
+    cuuint32_t bx[4] = {box[0], box[1], box[2], box[3]};
+    cuuint32_t es[4] = {1, 1, 1, 1};
+    CUresult r = encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, gdim, gstr, bx, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        swizzle64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                        CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        char b[96];
+        snprintf(b, sizeof b, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+        h->cuda_err = b;
+        return HYDRO_ECUDA;
+    }
+    return HYDRO_OK;
+}
+
+int setup_tma(hydro* h) {
+    const unsigned NF = (unsigned)h->nf;
+    const unsigned boxes[3][4] = {{TMA_CH, 32, 1, NF}, {32, TMA_CH, 1, NF}, {32, 1, TMA_CH, NF}};
+    int rc;
+    for (int d = 0; d < 3; ++d) {
+        unsigned b1[4] = {boxes[d][0], boxes[d][1], boxes[d][2], 1};
+        for (int b = 0; b < 3; ++b)
+            if ((rc = make_map(h, &h->mapU[b][d], h->buf[b], h->nf, boxes[d], d == 0)) != HYDRO_OK) return rc;
+        if ((rc = make_map(h, &h->mapW[d], h->W, 1, b1, d == 0)) != HYDRO_OK) return rc;
+        if ((rc = make_map(h, &h->mapP[d], h->P, 1, b1, d == 0)) != HYDRO_OK) return rc;
+    }
+    if ((rc = make_map(h, &h->mapL, h->L, h->nf, boxes[0], true)) != HYDRO_OK) return rc;
+    int bad = 0;
+    if (h->nf == 4) bad = set_smem_attr<0, 0, 4>() + set_smem_attr<1, 1, 4>() + set_smem_attr<2, 1, 4>() + set_smem_attr<2, 2, 4>();
+    else bad = set_smem_attr<0, 0, 5>() + set_smem_attr<1, 1, 5>() + set_smem_attr<2, 1, 5>() + set_smem_attr<2, 2, 5>();
+    if (bad) { h->cuda_err = "cudaFuncSetAttribute(max dynamic shared memory) failed"; return HYDRO_ECUDA; }
+    // march segments: one per line unless the grid is too small to fill the machine; multiples of the chunk
+    const int nd[3] = {h->nx, h->ny, h->nz};
+    for (int d = 0; d < 3; ++d) {
+        const long long nlane = d == 0 ? h->ny : h->nx;
+        const long long other = d == 2 ? h->ny : h->nz;
+        const long long blocks1 = ((nlane + 31) / 32) * other;
+        int seg = 1;
+        while (blocks1 * seg < (long long)h->num_sms * 3 && nd[d] / (seg * 2) >= 16) seg *= 2;
+        int ls = (nd[d] + seg - 1) / seg;
+        ls = (ls + TMA_CH - 1) / TMA_CH * TMA_CH;
+        h->seg_len[d] = ls;
+        h->tma_nseg[d] = (nd[d] + ls - 1) / ls;
+    }
+    return HYDRO_OK;
+}
+
 template <typename R, int DIR, int MODE>
 int launch_sweep(hydro* h, SweepArgs<R> a) {
+    if (h->use_tma && (h->tma_dirs >> DIR & 1)) return launch_sweep_tma<DIR, MODE>(h, a);
     const int nd = DIR == 0 ? h->nx : DIR == 1 ? h->ny : h->nz;
     const long long ntrans = h->N / nd;
     a.nseg = h->nseg[DIR];
@@ -141,7 +252,7 @@ int eval_stage(hydro* h, const void* Uin, int slot, int stage, double stage_c, b
     SweepArgs<R> a;
     a.U = (const R*)Uin; a.P = (const R*)h->P; a.W = (const R*)h->W; a.L = (R*)h->L;
     a.Un = (const R*)Un; a.Uout = (R*)Uout; a.diag = h->diag; a.slot = slot;
-    a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.nf = h->nf; a.nseg = 1; a.use_un = Un != 0;
+    a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.nf = h->nf; a.nseg = 1; a.use_un = Un != 0; a.seg_len = 0;
     a.N = h->N;
     a.eps_eff = (R)(144.0 * h->weno_eps);
     a.half_inv_dx = (R)(0.5 / h->dx);
@@ -253,6 +364,7 @@ int hydro_create(hydro_t** out, int nx, int ny, int nz, double dx, double dt, co
     h->cur = 0; h->L = h->P = h->W = h->scratch = 0; h->diag = 0; h->jets_dev = 0;
     h->jets_dirty = false; h->step = 0; h->prim_slot = 0; h->prims_valid = false; h->launches = 0;
     h->profiling = false;
+    h->use_tma = false;
     for (int k = 0; k < HYDRO_K_COUNT; ++k) { h->k_ms[k] = 0; h->k_n[k] = 0; }
     int rc = HYDRO_OK;
     do {
@@ -286,6 +398,12 @@ int hydro_create(hydro_t** out, int nx, int ny, int nz, double dx, double dt, co
             while (threads * seg < (long long)h->num_sms * 1024 && nd[d] / (seg * 2) >= 16) seg *= 2;
             h->nseg[d] = seg;
         }
+        // TMA-staged sweeps need 16-byte global strides (even nx in fp64); HYDRO_NO_TMA=1 forces the direct-load kernels
+        const char* no_tma = getenv("HYDRO_NO_TMA");
+        h->use_tma = o.precision == 64 && nx % 2 == 0 && !(no_tma && no_tma[0] == '1');
+        const char* td = getenv("HYDRO_TMA_DIRS");
+        h->tma_dirs = td ? atoi(td) : 7;
+        if (h->use_tma) rc = setup_tma(h);
     } while (0);
     if (rc != HYDRO_OK) {
         // keep the error text out of reach of the caller: handle is destroyed

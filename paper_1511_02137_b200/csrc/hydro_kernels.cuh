@@ -302,6 +302,7 @@ struct SweepArgs {
     const Diag* diag;
     int slot;        // which DiagSlot holds alpha of U_s
     int nx, ny, nz, nf, nseg, use_un;
+    int seg_len;     // TMA sweeps: march cells per block (multiple of 8)
     long long N;
     R eps_eff;       // 144 * weno_eps: the split fluxes are carried as 2 f^+-, beta is carried as 36 beta
     R half_inv_dx;   // 0.5 / dx

@@ -105,7 +105,8 @@ def test_con2prim_parity(H, oracle):
 
 
 # ------------------------------------------------------------------------------------------------ a-3..a-5, a-7
-@pytest.mark.parametrize("n", [(32, 32, 32), (37, 19, 23), (7, 5, 3), (1, 1, 40), (130, 9, 6)])
+@pytest.mark.parametrize("n", [(32, 32, 32), (37, 19, 23), (7, 5, 3), (1, 1, 40), (130, 9, 6), (34, 19, 23), (2, 3, 4),
+                               (64, 40, 72), (8, 100, 8), (72, 8, 33)])
 @pytest.mark.parametrize("nf", [4, 5])
 def test_rhs_single_stage_parity(H, oracle, n, nf):
     c = S.scaled_config(0, n)
