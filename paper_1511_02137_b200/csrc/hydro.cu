@@ -2,7 +2,7 @@
 // No CPU fallback: every step of the path runs in the kernels of hydro_kernels.cuh.
 #include "../../include/hydro.h"
 #include "hydro_kernels.cuh"
-#include "hydro_sweep_tma.cuh"
+#include "hydro_sweep_ring.cuh"
 
 #include <cudaTypedefs.h>
 
@@ -37,10 +37,9 @@ struct hydro {
     int prim_slot;                      // DiagSlot holding alpha of buf[cur]'s primitives
     bool prims_valid;
     int nseg[3];
-    // TMA sweeps (fp64, even nx): tensor maps per state copy and direction, march cells per block
+    // ring sweeps (fp64, even nx): tensor maps per buffer and direction, march cells per block
     bool use_tma;
-    int tma_dirs;                       // bit d: direction d uses the TMA sweep (HYDRO_TMA_DIRS, default 7)
-    CUtensorMap mapU[3][3], mapW[3], mapP[3], mapL;
+    CUtensorMap mapU[3][3], mapW[3], mapP[3], mapL[3];
     int seg_len[3], tma_nseg[3];
     int num_sms;
     long long launches;
@@ -122,39 +121,47 @@ int buf_index(const hydro* h, const void* U) {
     return -1;
 }
 
-template <int DIR, int MODE, int NF>
-int launch_sweep_tma_nf(hydro* h, const SweepArgs<double>& a0) {
-    SweepArgs<double> a = a0;
-    const int b = buf_index(h, a.U);
+// One ring sweep (hydro_sweep_ring.cuh).  `Us` must be one of the three state buffers; `out_map` is the tensor map
+// (for direction DIR) of the buffer the result is stored / reduced into; `un_map` that of U^n (OUT_COMBINE).
+template <int DIR, int OUT, int NF>
+int launch_ring_nf(hydro* h, const void* Us, int slot, const CUtensorMap* out_map, const CUtensorMap* un_map, double coef,
+                   double rk_a, double rk_b) {
+    const int b = buf_index(h, Us);
     if (b < 0) return HYDRO_ESTATE;
-    SweepMaps m;
-    m.U = h->mapU[b][DIR]; m.W = h->mapW[DIR]; m.P = h->mapP[DIR]; m.Lst = h->mapL;
-    a.seg_len = h->seg_len[DIR];
+    RingMaps m;
+    m.U = h->mapU[b][DIR]; m.W = h->mapW[DIR]; m.P = h->mapP[DIR]; m.Out = *out_map; m.Un = un_map ? *un_map : *out_map;
+    RingArgs a;
+    a.diag = h->diag; a.slot = slot; a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.seg_len = h->seg_len[DIR];
+    a.eps_eff = 144.0 * h->weno_eps; a.coef = coef; a.dt = h->dt; a.rk_a = rk_a; a.rk_b = rk_b;
     const int nlane = DIR == 0 ? h->ny : h->nx;
     const int other = DIR == 2 ? h->ny : h->nz;
     dim3 grid((unsigned)(((nlane + 31) / 32) * other), (unsigned)h->tma_nseg[DIR], 1);
     dim3 block(32, NF, 1);
-    const int smem = sweep_tma_smem_bytes(NF, DIR, 8);
     {
         Timer t(h, HYDRO_K_SWEEP_X + DIR);
-        k_sweep_tma<DIR, MODE, NF><<<grid, block, smem, h->stream>>>(m, a);
+        k_sweep_ring<DIR, OUT, NF><<<grid, block, ring_smem_bytes(NF, OUT), h->stream>>>(m, a);
     }
     h->launches += 1;
     CK(cudaGetLastError());
     return HYDRO_OK;
 }
 
-template <int DIR, int MODE>
-int launch_sweep_tma(hydro* h, const SweepArgs<double>& a) {
-    return h->nf == 4 ? launch_sweep_tma_nf<DIR, MODE, 4>(h, a) : launch_sweep_tma_nf<DIR, MODE, 5>(h, a);
+template <int DIR, int OUT>
+int launch_ring(hydro* h, const void* Us, int slot, const CUtensorMap* out_map, const CUtensorMap* un_map, double coef,
+                double rk_a, double rk_b) {
+    return h->nf == 4 ? launch_ring_nf<DIR, OUT, 4>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b)
+                      : launch_ring_nf<DIR, OUT, 5>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b);
 }
-template <int DIR, int MODE>
-int launch_sweep_tma(hydro*, const SweepArgs<float>&) { return HYDRO_ESTATE; }
 
-template <int DIR, int MODE, int NF>
+template <int DIR, int OUT, int NF>
 int set_smem_attr() {
-    return cudaFuncSetAttribute(k_sweep_tma<DIR, MODE, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                sweep_tma_smem_bytes(NF, DIR, 8)) == cudaSuccess ? 0 : 1;
+    return cudaFuncSetAttribute(k_sweep_ring<DIR, OUT, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                ring_smem_bytes(NF, OUT)) == cudaSuccess ? 0 : 1;
+}
+template <int NF>
+int set_smem_attrs() {
+    return set_smem_attr<0, OUT_STORE, NF>() + set_smem_attr<0, OUT_COMBINE1, NF>() + set_smem_attr<0, OUT_COMBINE, NF>() +
+           set_smem_attr<1, OUT_REDUCE, NF>() + set_smem_attr<2, OUT_REDUCE, NF>();
 }
 
 // 4-D tensor map (x, y, z, field) of one SoA buffer with `nfb` fields; box given per dimension
@@ -188,7 +195,7 @@ int make_map(hydro* h, CUtensorMap* out, void* base, int nfb, const unsigned box
 
 int setup_tma(hydro* h) {
     const unsigned NF = (unsigned)h->nf;
-    const unsigned boxes[3][4] = {{TMA_CH, 32, 1, NF}, {32, TMA_CH, 1, NF}, {32, 1, TMA_CH, NF}};
+    const unsigned boxes[3][4] = {{RING_CH, 32, 1, NF}, {32, RING_CH, 1, NF}, {32, 1, RING_CH, NF}};
     int rc;
     for (int d = 0; d < 3; ++d) {
         unsigned b1[4] = {boxes[d][0], boxes[d][1], boxes[d][2], 1};
@@ -196,12 +203,12 @@ int setup_tma(hydro* h) {
             if ((rc = make_map(h, &h->mapU[b][d], h->buf[b], h->nf, boxes[d], d == 0)) != HYDRO_OK) return rc;
         if ((rc = make_map(h, &h->mapW[d], h->W, 1, b1, d == 0)) != HYDRO_OK) return rc;
         if ((rc = make_map(h, &h->mapP[d], h->P, 1, b1, d == 0)) != HYDRO_OK) return rc;
+        if ((rc = make_map(h, &h->mapL[d], h->L, h->nf, boxes[d], d == 0)) != HYDRO_OK) return rc;
     }
-    if ((rc = make_map(h, &h->mapL, h->L, h->nf, boxes[0], true)) != HYDRO_OK) return rc;
-    int bad = 0;
-    if (h->nf == 4) bad = set_smem_attr<0, 0, 4>() + set_smem_attr<1, 1, 4>() + set_smem_attr<2, 1, 4>() + set_smem_attr<2, 2, 4>();
-    else bad = set_smem_attr<0, 0, 5>() + set_smem_attr<1, 1, 5>() + set_smem_attr<2, 1, 5>() + set_smem_attr<2, 2, 5>();
-    if (bad) { h->cuda_err = "cudaFuncSetAttribute(max dynamic shared memory) failed"; return HYDRO_ECUDA; }
+    if (h->nf == 4 ? set_smem_attrs<4>() : set_smem_attrs<5>()) {
+        h->cuda_err = "cudaFuncSetAttribute(max dynamic shared memory) failed";
+        return HYDRO_ECUDA;
+    }
     // march segments: one per line unless the grid is too small to fill the machine; multiples of the chunk
     const int nd[3] = {h->nx, h->ny, h->nz};
     for (int d = 0; d < 3; ++d) {
@@ -211,7 +218,7 @@ int setup_tma(hydro* h) {
         int seg = 1;
         while (blocks1 * seg < (long long)h->num_sms * 3 && nd[d] / (seg * 2) >= 16) seg *= 2;
         int ls = (nd[d] + seg - 1) / seg;
-        ls = (ls + TMA_CH - 1) / TMA_CH * TMA_CH;
+        ls = (ls + RING_CH - 1) / RING_CH * RING_CH;
         h->seg_len[d] = ls;
         h->tma_nseg[d] = (nd[d] + ls - 1) / ls;
     }
@@ -220,7 +227,6 @@ int setup_tma(hydro* h) {
 
 template <typename R, int DIR, int MODE>
 int launch_sweep(hydro* h, SweepArgs<R> a) {
-    if (h->use_tma && (h->tma_dirs >> DIR & 1)) return launch_sweep_tma<DIR, MODE>(h, a);
     const int nd = DIR == 0 ? h->nx : DIR == 1 ? h->ny : h->nz;
     const long long ntrans = h->N / nd;
     a.nseg = h->nseg[DIR];
@@ -245,10 +251,51 @@ int upload_jets(hydro* h) {
     return HYDRO_OK;
 }
 
-// L(U_in, t_n + stage_c dt) into h->L; if Uout != 0 the last sweep also forms the next stage state.
+template <typename R>
+int launch_source(hydro* h, int slot, int stage, double stage_c, bool commit, double rk_weight, void* target, double scale) {
+    int rc;
+    if ((rc = upload_jets<R>(h)) != HYDRO_OK) return rc;
+    SourceArgs s;
+    s.diag = h->diag; s.jets = h->jets_dev; s.njets = (int)h->jets.size(); s.slot = slot; s.stage = stage;
+    s.commit = commit ? 1 : 0; s.nx = h->nx; s.ny = h->ny; s.nz = h->nz; s.N = h->N; s.step = h->step;
+    s.stage_c = stage_c; s.dx = h->dx; s.dt = h->dt; s.rk_weight = rk_weight; s.scale = scale;
+    {
+        Timer t(h, HYDRO_K_SOURCE);
+        k_source<R><<<1, 32, 0, h->stream>>>(s, (const R*)h->P, (R*)target);
+    }
+    h->launches += 1;
+    CK(cudaGetLastError());
+    return HYDRO_OK;
+}
+
+// Ring path (fp64, even nx).  With Uout: the x sweep stores U_next = a U^n + b (U_s + dt L_x), the source kernel and
+// the y, z sweeps add b dt S, b dt L_y, b dt L_z to it (the stage update is linear in L).  Without: L into h->L.
+int eval_stage_ring(hydro* h, const void* Uin, int slot, int stage, double stage_c, bool commit, double rk_weight,
+                    void* Uout, const void* Un, double rk_a, double rk_b) {
+    const double hid = 0.5 / h->dx;
+    int rc;
+    if (Uout) {
+        const int bo = buf_index(h, Uout), bn = Un ? buf_index(h, Un) : -1;
+        if (bo < 0 || (Un && bn < 0)) return HYDRO_ESTATE;
+        if (Un) rc = launch_ring<0, OUT_COMBINE>(h, Uin, slot, &h->mapU[bo][0], &h->mapU[bn][0], hid, rk_a, rk_b);
+        else rc = launch_ring<0, OUT_COMBINE1>(h, Uin, slot, &h->mapU[bo][0], 0, hid, 0.0, 1.0);
+        if (rc != HYDRO_OK) return rc;
+        const double bdt = (Un ? rk_b : 1.0) * h->dt;
+        if ((rc = launch_source<double>(h, slot, stage, stage_c, commit, rk_weight, Uout, bdt)) != HYDRO_OK) return rc;
+        if ((rc = launch_ring<1, OUT_REDUCE>(h, Uin, slot, &h->mapU[bo][1], 0, bdt * hid, 0.0, 0.0)) != HYDRO_OK) return rc;
+        return launch_ring<2, OUT_REDUCE>(h, Uin, slot, &h->mapU[bo][2], 0, bdt * hid, 0.0, 0.0);
+    }
+    if ((rc = launch_ring<0, OUT_STORE>(h, Uin, slot, &h->mapL[0], 0, hid, 0.0, 0.0)) != HYDRO_OK) return rc;
+    if ((rc = launch_source<double>(h, slot, stage, stage_c, commit, rk_weight, h->L, 1.0)) != HYDRO_OK) return rc;
+    if ((rc = launch_ring<1, OUT_REDUCE>(h, Uin, slot, &h->mapL[1], 0, hid, 0.0, 0.0)) != HYDRO_OK) return rc;
+    return launch_ring<2, OUT_REDUCE>(h, Uin, slot, &h->mapL[2], 0, hid, 0.0, 0.0);
+}
+
+// L(U_in, t_n + stage_c dt) into h->L; if Uout != 0 the stage combination forms the next stage state.
 template <typename R>
 int eval_stage(hydro* h, const void* Uin, int slot, int stage, double stage_c, bool commit, double rk_weight,
                void* Uout, const void* Un, double rk_a, double rk_b) {
+    if (h->use_tma) return eval_stage_ring(h, Uin, slot, stage, stage_c, commit, rk_weight, Uout, Un, rk_a, rk_b);
     SweepArgs<R> a;
     a.U = (const R*)Uin; a.P = (const R*)h->P; a.W = (const R*)h->W; a.L = (R*)h->L;
     a.Un = (const R*)Un; a.Uout = (R*)Uout; a.diag = h->diag; a.slot = slot;
@@ -260,17 +307,7 @@ int eval_stage(hydro* h, const void* Uin, int slot, int stage, double stage_c, b
     int rc;
     if ((rc = launch_sweep<R, 0, 0>(h, a)) != HYDRO_OK) return rc;
     if ((rc = launch_sweep<R, 1, 1>(h, a)) != HYDRO_OK) return rc;
-    if ((rc = upload_jets<R>(h)) != HYDRO_OK) return rc;
-    SourceArgs s;
-    s.diag = h->diag; s.jets = h->jets_dev; s.njets = (int)h->jets.size(); s.slot = slot; s.stage = stage;
-    s.commit = commit ? 1 : 0; s.nx = h->nx; s.ny = h->ny; s.nz = h->nz; s.N = h->N; s.step = h->step;
-    s.stage_c = stage_c; s.dx = h->dx; s.dt = h->dt; s.rk_weight = rk_weight;
-    {
-        Timer t(h, HYDRO_K_SOURCE);
-        k_source<R><<<1, 32, 0, h->stream>>>(s, (const R*)h->P, (R*)h->L);
-    }
-    h->launches += 1;
-    CK(cudaGetLastError());
+    if ((rc = launch_source<R>(h, slot, stage, stage_c, commit, rk_weight, h->L, 1.0)) != HYDRO_OK) return rc;
     if (Uout) rc = launch_sweep<R, 2, 2>(h, a);
     else rc = launch_sweep<R, 2, 1>(h, a);
     return rc;
@@ -401,8 +438,6 @@ int hydro_create(hydro_t** out, int nx, int ny, int nz, double dx, double dt, co
         // TMA-staged sweeps need 16-byte global strides (even nx in fp64); HYDRO_NO_TMA=1 forces the direct-load kernels
         const char* no_tma = getenv("HYDRO_NO_TMA");
         h->use_tma = o.precision == 64 && nx % 2 == 0 && !(no_tma && no_tma[0] == '1');
-        const char* td = getenv("HYDRO_TMA_DIRS");
-        h->tma_dirs = td ? atoi(td) : 7;
         if (h->use_tma) rc = setup_tma(h);
     } while (0);
     if (rc != HYDRO_OK) {

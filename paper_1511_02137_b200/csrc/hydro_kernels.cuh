@@ -421,6 +421,7 @@ struct SourceArgs {
     int nx, ny, nz;
     long long N, step;
     double stage_c, dx, dt, rk_weight;
+    double scale;                      // the deposit is added to `target` times this (1 for L, b dt for a stage state)
 };
 
 __device__ __forceinline__ int jet_axis_index(double x, int n, double dx) {
@@ -432,7 +433,7 @@ __device__ __forceinline__ int jet_axis_index(double x, int n, double dx) {
 }
 
 template <typename R>
-__global__ void k_source(SourceArgs a, const R* __restrict__ P, R* __restrict__ L) {
+__global__ void k_source(SourceArgs a, const R* __restrict__ P, R* __restrict__ L /* target */) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     Diag* dg = a.diag;
     const DiagSlot* s = &dg->slot[a.slot];
@@ -458,7 +459,7 @@ __global__ void k_source(SourceArgs a, const R* __restrict__ P, R* __restrict__ 
             const double T2 = sqrt(e_c / (G_DOF * HBARC));       // T^2, T in 1/fm
             const double T = sqrt(T2);
             q = HBARC * jt.crcf * (jt.k_rad * T2 * T * ell + jt.k_coll * T2);
-            const double r = q / dx3;
+            const double r = a.scale * (q / dx3);
             L[c] += (R)r;
             L[a.N + c] += (R)(r * jt.nx);
             L[2 * a.N + c] += (R)(r * jt.ny);

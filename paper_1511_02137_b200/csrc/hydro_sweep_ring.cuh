@@ -1,0 +1,434 @@
+// hydro_sweep_ring.cuh -- the WENO7-LF sweep kernels of the hot path (sm_100a, fp64).  PRODUCT.
+//
+// Steps a-3 (WENO7 reconstruction of the Lax-Friedrichs split fluxes), a-4 (flux divergence,
+// eq. 1), a-6 (SSP-RK3 stage combination) and a-7 (outflow ghosts) of SURVEY.md 8(a), organised
+// around the one resource that bounds them, the FP64 pipe:
+//
+//   block   = 32 lanes x NF field-warps.  The lanes are 32 neighbouring grid lines (consecutive x for the y/z
+//             sweeps, consecutive y for the x sweep); warp f reconstructs conserved field f, so the warps of a
+//             block share every input row: U (all fields), W = scale/(E+p) and P.
+//   input   = a ring of RING_NSTAGE shared-memory stages, each CH = 8 march cells x 32 lanes of (U[NF], W, P),
+//             filled by one thread with cp.async.bulk.tensor (TMA) box loads that complete on an mbarrier, one
+//             chunk ahead of the arithmetic.  The x sweep uses the 64-byte TMA swizzle so that lane = row reads
+//             its own row with a 2-way bank conflict at most.
+//   window  = every thread marches along the sweep axis and keeps, per split sign, the undivided differences of
+//             the last cells in ROTATING registers: slot = march cell mod 8, all indices compile-time constants
+//             in a fully unrolled 8-row chunk body, so the window never moves through registers and the body has
+//             no branches (r1_b profile: 45-50 % of the issued instructions of the previous kernel were moves).
+//   ghosts  = TMA zero-fills out-of-range cells; in the (at most two) chunks of a line that hold ghost rows the
+//             zero rows are overwritten in shared memory with the edge cell's row (zero-gradient outflow, R8b).
+//   output  = a shared-memory tile per chunk, written back with ONE TMA op per chunk:
+//               OUT_STORE     L        = c (F_{i-1/2} - F_{i+1/2})                    tensor store
+//               OUT_REDUCE    target  += c (F_{i-1/2} - F_{i+1/2})                    tensor reduce-add (in L2)
+//               OUT_COMBINE1  U_next   = U_s + dt L_x                                 tensor store   (stage 1)
+//               OUT_COMBINE   U_next   = a U^n + b (U_s + dt L_x)                     tensor store   (stages 2, 3)
+//             The stage update is linear in L = L_x + L_y + L_z + S, so the x sweep writes the combined state with
+//             its own part and the y and z sweeps (and the source kernel) add b dt L_y, b dt L_z (b dt S) to it.
+//             No thread ever waits on a global load or store; out-of-range rows and lanes are clipped by TMA.
+#pragma once
+#include <cuda.h>
+#include "hydro_kernels.cuh"
+
+namespace hydro_dev {
+
+constexpr int RING_CH = 8;                 // march cells per chunk
+constexpr int RING_NSTAGE = 3;             // input ring depth: chunks m-1 (still read), m (current), m+1 (in flight)
+constexpr int RING_SUB = RING_CH * 32;     // reals per sub-tile (one field, one chunk)
+
+enum { OUT_STORE = 0, OUT_REDUCE = 1, OUT_COMBINE1 = 2, OUT_COMBINE = 3 };
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// Bounded wait: a TMA load that never completes (bad tensor map) must become a CUDA error, not a hung GPU.
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    const uint32_t addr = smem_u32(bar);
+    for (unsigned spin = 0; spin < (1u << 22); ++spin) {
+        uint32_t done;
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(done)
+            : "r"(addr), "r"(parity)
+            : "memory");
+        if (done) return;
+    }
+    __trap();
+}
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2,
+                                            int c3) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+        : "memory");
+}
+__device__ __forceinline__ void tma_store_4d(const CUtensorMap* tm, const void* src, int c0, int c1, int c2, int c3) {
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5}], [%1];" ::"l"(tm),
+                 "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+                 : "memory");
+}
+__device__ __forceinline__ void tma_reduce_add_4d(const CUtensorMap* tm, const void* src, int c0, int c1, int c2,
+                                                  int c3) {
+    asm volatile("cp.reduce.async.bulk.tensor.4d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3, %4, %5}], [%1];" ::"l"(tm),
+                 "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+                 : "memory");
+}
+__device__ __forceinline__ void tma_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void tma_wait_all0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// shared-memory plan of one launch (host and device agree through these functions); units: reals
+__host__ __device__ constexpr int ring_stage_reals(int nf) { return (nf + 2) * RING_SUB; }
+__host__ __device__ constexpr int ring_smem_bytes(int nf, int out) {
+    return (RING_NSTAGE * ring_stage_reals(nf)            // input ring
+            + 2 * nf * RING_SUB                            // two output tiles
+            + (out == OUT_COMBINE ? 2 * nf * RING_SUB : 0) // two U^n tiles
+            + RING_SUB) * 8                                // one tile of zeros
+           + 64;                                           // mbarriers
+}
+
+struct RingMaps {
+    CUtensorMap U, W, P;       // loads: stage state (NF fields per box), W and P (one field per box)
+    CUtensorMap Un;            // load : U^n at the output cells (OUT_COMBINE)
+    CUtensorMap Out;           // store / reduce target (NF fields per box)
+};
+
+struct RingArgs {
+    const Diag* diag;
+    int slot;                  // which DiagSlot holds alpha of U_s
+    int nx, ny, nz;
+    int seg_len;               // march cells per block (multiple of RING_CH)
+    double eps_eff;            // 144 * weno_eps: the split fluxes are carried as 2 f^+-, beta as 36 beta
+    double coef;               // OUT_STORE / OUT_REDUCE: c = [b dt] / (2 dx);  OUT_COMBINE*: 1 / (2 dx)
+    double dt, rk_a, rk_b;
+};
+
+// element offset inside a sub-tile of march row r (0..7) for this lane
+template <int DIR>
+__device__ __forceinline__ int sub_off(int r, int lane) {
+    if (DIR == 0) {
+        // dense box layout (8 cells of x fastest, 32 rows): byte = lane*64 + r*8, TMA 64-byte swizzle:
+        // 16-byte chunk index (bits 4..5) ^= address bits 7..8 = (lane >> 1) & 3
+        return lane * 8 + ((((r >> 1) ^ ((lane >> 1) & 3)) << 1) | (r & 1));
+    }
+    return r * 32 + lane;
+}
+
+// ------------------------------------------------------------------------------------------------ rotating window
+// Undivided differences of one split flux along the march, slot = march row mod 8:
+//   V = value, D = V - V_prev, E = D - D_prev, T = E - E_prev (only the newest is kept), G = T - T_prev,
+//   S = C3 T^2 + eps.  Live at any time: 4 V, 6 D, 5 E, 4 S, 3 G, 1 T (the other slots are dead registers).
+struct RotWin {
+    double V[8], D[8], E[8], S[8], G[8], T;
+    __device__ __forceinline__ void clear() {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) { V[j] = 0.0; D[j] = 0.0; E[j] = 0.0; S[j] = 0.0; G[j] = 0.0; }
+        T = 0.0;
+    }
+};
+
+template <int r>
+__device__ __forceinline__ void rot_push(RotWin& w, double x, double c3, double eps) {
+    constexpr int p = (r + 7) & 7;
+    const double dn = x - w.V[p];
+    const double en = dn - w.D[p];
+    const double tn = en - w.E[p];
+    w.G[r] = tn - w.T;
+    w.S[r] = fma(c3 * tn, tn, eps);
+    w.V[r] = x;
+    w.D[r] = dn;
+    w.E[r] = en;
+    w.T = tn;
+}
+
+// One WENO7-JS reconstruction (r = 4) from the 1st..4th undivided differences in stencil order (D_j, E_j, G_j) and
+// S_j = 39.05 T_j^2 + eps (formulas: DESIGN.md "WENO7 in difference form"):
+//   candidates   12 (q_0 - x_c) = 3 D_0 - 10 D_1 + 13 D_2,  12 (q_1-q_0) = 3 G_0,  12 (q_2-q_1) = -G_1,  12 (q_3-q_2) = G_2
+//   smoothness   36 beta_k + eps = lam_k^2 + 39 m_k^2 + S_k,
+//                lam_0 = 2 D_0 - 7 D_1 + 11 D_2, lam_1 = lam_0 + 2 G_0, lam_2 = lam_1 - G_1, lam_3 = lam_2 + 2 G_2,
+//                m_0 = 2 E_1 - E_0,  m_1 = m_2 = E_2,  m_3 = 2 E_3 - E_4
+//   weights      omega_k ~ d_k prod_{j != k} (eps + beta_j)^2,  d = (1, 12, 18, 4)/35  (common denominator; range-safe
+//                in fp64)
+// Returns base12 = 12 (q_0 - x_c) and num12/den = 12 sum_k omega_k (q_k - q_0):  W = x_c + (base12 + num12/den)/12.
+__device__ __forceinline__ void weno7_diff(double D0, double D1, double D2, double E0, double E1, double E2, double E3,
+                                           double E4, double S0, double S1, double S2, double S3, double G0, double G1,
+                                           double G2, double& base12, double& num12, double& den) {
+    const double lam0 = fma(11.0, D2, fma(-7.0, D1, 2.0 * D0));
+    const double lam1 = fma(2.0, G0, lam0);
+    const double lam2 = lam1 - G1;
+    const double lam3 = fma(2.0, G2, lam2);
+    const double m0 = fma(2.0, E1, -E0);
+    const double m3 = fma(2.0, E3, -E4);
+    const double e39 = 39.0 * E2;
+    const double b0 = fma(lam0, lam0, fma(39.0 * m0, m0, S0));
+    const double b1 = fma(lam1, lam1, fma(e39, E2, S1));
+    const double b2 = fma(lam2, lam2, fma(e39, E2, S2));
+    const double b3 = fma(lam3, lam3, fma(39.0 * m3, m3, S3));
+    const double t0 = b0 * b0, t1 = b1 * b1, t2 = b2 * b2, t3 = b3 * b3;
+    const double p01 = t0 * t1, p23 = t2 * t3;
+    const double u0 = t1 * p23, u1 = t0 * p23, u2 = t3 * p01, u3 = t2 * p01;
+    const double a3 = 4.0 * u3;
+    const double a23 = fma(18.0, u2, a3);
+    const double a123 = fma(12.0, u1, a23);
+    den = u0 + a123;
+    num12 = fma(a123, 3.0 * G0, fma(-a23, G1, a3 * G2));
+    base12 = fma(13.0, D2, fma(-10.0, D1, 3.0 * D0));
+}
+
+// reciprocal of a normal, well-scaled double: hardware seed (the upper 32 bits of the operand and of the result,
+// i.e. a relative error e of about 2^-20) + one cubic step r (1 + e + e^2), error e^3 ~ 2^-60
+__device__ __forceinline__ double rcp_cubic(double x) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    const double e = fma(-x, r, 1.0);
+    const double t = fma(e, e, e);
+    return fma(r, t, r);
+}
+
+// 2 F_hat at the interface whose newest needed cell sits in slot r of both windows (plus side lags one slot):
+//   plus  side: cells i-3..i+3 = slots r-7..r-1, centre i   = V[r-4]
+//   minus side: cells i-2..i+4 = slots r-6..r,   centre i+1 = V[r-3], stencil order reversed (D_j = -d[5-j], ...)
+template <int r>
+__device__ __forceinline__ double rot_flux(const RotWin& wp, const RotWin& wm) {
+#define SL(k) (((r) + (k) + 16) & 7)
+    double bp, np_, dp, bm, nm, dm;
+    weno7_diff(wp.D[SL(-6)], wp.D[SL(-5)], wp.D[SL(-4)],
+               wp.E[SL(-5)], wp.E[SL(-4)], wp.E[SL(-3)], wp.E[SL(-2)], wp.E[SL(-1)],
+               wp.S[SL(-4)], wp.S[SL(-3)], wp.S[SL(-2)], wp.S[SL(-1)],
+               wp.G[SL(-3)], wp.G[SL(-2)], wp.G[SL(-1)], bp, np_, dp);
+    weno7_diff(-wm.D[SL(0)], -wm.D[SL(-1)], -wm.D[SL(-2)],
+               wm.E[SL(0)], wm.E[SL(-1)], wm.E[SL(-2)], wm.E[SL(-3)], wm.E[SL(-4)],
+               wm.S[SL(0)], wm.S[SL(-1)], wm.S[SL(-2)], wm.S[SL(-3)],
+               wm.G[SL(0)], wm.G[SL(-1)], wm.G[SL(-2)], bm, nm, dm);
+    const double x = fma(np_, dm, nm * dp) * rcp_cubic(dp * dm);
+    return fma((bp + bm) + x, 1.0 / 12.0, wp.V[SL(-4)] + wm.V[SL(-3)]);
+#undef SL
+}
+
+// per-thread view of one input stage: byte-free element pointers with the lane offset folded in
+template <int DIR>
+struct RowPtr {
+    const double* q[DIR == 0 ? 4 : 1];     // DIR 0: one pointer per swizzle class (r >> 1)
+    __device__ __forceinline__ void set(const double* tile, int lane) {
+        if (DIR == 0) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) q[k] = tile + lane * 8 + ((k ^ ((lane >> 1) & 3)) << 1);
+        } else q[0] = tile + lane;
+    }
+    template <int r>
+    __device__ __forceinline__ double at() const {
+        if (DIR == 0) return q[r >> 1][r & 1];
+        return q[0][r * 32];
+    }
+};
+
+template <int DIR, int OUT, int NF>
+struct SweepCtx {
+    RotWin wp, wm;
+    double fhat_prev;
+    double alpha, c3, eps, coef, dt, rk_a, rk_b, kE;
+    // current chunk
+    RowPtr<DIR> pu, pmd, pa, pw, pp;       // own field, normal momentum, A operand, W (or zeros), P (or zeros)
+    RowPtr<DIR> pus[2];                    // U_s of the output cells: rows 4..7 of the previous chunk, 0..3 of this one
+    RowPtr<DIR> pun;                       // U^n of the output cells
+    double* out;                           // this field's output sub-tile, lane offset NOT folded in
+    int lane;
+
+    // split fluxes of the row's cell, carried as 2 f^+- = F +- alpha U:
+    //   F^d_E = M_d;  F^d_{M_j} = M_j v_d + p delta_jd;  F^d_{N_B} = N_B v_d;  v_d = M_d * W   (a-3)
+    // written branch-free as F = A * B + C with per-warp operand tiles: energy A = M_d, B = 1, C = 0;
+    // momenta / N_B: A = U_f, B = M_d W, C = p (normal component) or 0.
+    template <int r>
+    __device__ __forceinline__ void load_push() {
+        const double u = pu.template at<r>();
+        const double md = pmd.template at<r>();
+        const double B = fma(md, pw.template at<r>(), kE);
+        const double F = fma(pa.template at<r>(), B, pp.template at<r>());
+        rot_push<r>(wp, fma(alpha, u, F), c3, eps);
+        rot_push<r>(wm, fma(-alpha, u, F), c3, eps);
+    }
+    template <int r>
+    __device__ __forceinline__ void emit() {
+        const double fhat = rot_flux<r>(wp, wm);
+        const double mdiv = (fhat_prev - fhat) * coef;
+        fhat_prev = fhat;
+        double o;
+        if (OUT == OUT_STORE || OUT == OUT_REDUCE) o = mdiv;
+        else {
+            // output cell i = (row's cell) - 4: U_s from the ring, row (r + 4) & 7 of the previous / this chunk
+            const double us = pus[r < 4 ? 0 : 1].template at<(r + 4) & 7>();
+            o = fma(dt, mdiv, us);
+            if (OUT == OUT_COMBINE) o = fma(rk_b, o, rk_a * pun.template at<r>());
+        }
+        out[sub_off<DIR>(r, lane)] = o;
+    }
+    template <int r>
+    __device__ __forceinline__ void row() {
+        load_push<r>();
+        emit<r>();
+    }
+};
+
+template <int DIR, int OUT, int NF>
+__global__ void __launch_bounds__(32 * NF, NF == 4 ? 3 : 2)
+k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
+    typedef double R;
+    // 1024-byte alignment: the swizzle pattern is a function of the absolute shared address
+    extern __shared__ __align__(1024) unsigned char smem[];
+    constexpr int STAGE_REALS = ring_stage_reals(NF);
+    constexpr uint32_t STAGE_BYTES = STAGE_REALS * sizeof(R);
+    constexpr uint32_t UN_BYTES = NF * RING_SUB * sizeof(R);
+    R* stages = (R*)smem;
+    R* outt = stages + RING_NSTAGE * STAGE_REALS;                      // two output tiles of NF sub-tiles
+    R* unt = outt + 2 * NF * RING_SUB;                                 // OUT_COMBINE: two U^n tiles
+    R* zeros = unt + (OUT == OUT_COMBINE ? 2 * NF * RING_SUB : 0);
+    uint64_t* full = (uint64_t*)(zeros + RING_SUB);
+
+    const int lane = threadIdx.x, f = threadIdx.y;
+    const bool leader = (lane == 0 && f == 0);
+    const int nd = DIR == 0 ? a.nx : DIR == 1 ? a.ny : a.nz;
+
+    // transverse tile of 32 lines and the march segment of this block
+    int t0, tfix;                  // first transverse index along the lane axis, fixed transverse index
+    {
+        const int nlane_axis = DIR == 0 ? a.ny : a.nx;
+        const int tiles = (nlane_axis + 31) >> 5;
+        const int tb = blockIdx.x % tiles;
+        tfix = blockIdx.x / tiles;
+        t0 = tb << 5;
+    }
+    const int s0 = blockIdx.y * a.seg_len;
+    if (s0 >= nd) return;          // whole block exits together
+    const int len = min(nd, s0 + a.seg_len) - s0;
+    const int nchunks = (len + RING_CH - 1) / RING_CH + 1;             // chunk m holds cells s0 - 4 + 8m .. + 7
+
+    if (leader) {
+#pragma unroll
+        for (int s = 0; s < RING_NSTAGE; ++s) mbar_init(&full[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int i = f * 32 + lane; i < RING_SUB; i += 32 * NF) zeros[i] = 0.0;
+    __syncthreads();
+
+    auto coords = [&](int cm, int& c0, int& c1, int& c2) {
+        if (DIR == 0) { c0 = cm; c1 = t0; c2 = tfix; }
+        else if (DIR == 1) { c0 = t0; c1 = cm; c2 = tfix; }
+        else { c0 = t0; c1 = tfix; c2 = cm; }
+    };
+    auto issue = [&](int m) {                                          // leader only
+        const int st = m % RING_NSTAGE;
+        R* dst = stages + st * STAGE_REALS;
+        int c0, c1, c2;
+        coords(s0 - 4 + m * RING_CH, c0, c1, c2);
+        const bool with_un = (OUT == OUT_COMBINE) && m > 0;
+        mbar_expect_tx(&full[st], STAGE_BYTES + (with_un ? UN_BYTES : 0u));
+        tma_load_4d(dst, &maps.U, &full[st], c0, c1, c2, 0);
+        tma_load_4d(dst + NF * RING_SUB, &maps.W, &full[st], c0, c1, c2, 0);
+        tma_load_4d(dst + (NF + 1) * RING_SUB, &maps.P, &full[st], c0, c1, c2, 0);
+        if (with_un) {
+            coords(s0 + (m - 1) * RING_CH, c0, c1, c2);                // the cells chunk m emits
+            tma_load_4d(unt + (m & 1) * NF * RING_SUB, &maps.Un, &full[st], c0, c1, c2, 0);
+        }
+    };
+    auto flush = [&](int m) {                                          // leader only: write back chunk m's outputs
+        int c0, c1, c2;
+        coords(s0 + (m - 1) * RING_CH, c0, c1, c2);
+        const R* src = outt + (m & 1) * NF * RING_SUB;
+        if (OUT == OUT_REDUCE) tma_reduce_add_4d(&maps.Out, src, c0, c1, c2, 0);
+        else tma_store_4d(&maps.Out, src, c0, c1, c2, 0);
+        tma_commit();
+    };
+    if (leader) {
+        issue(0);
+        if (nchunks > 1) issue(1);
+    }
+
+    SweepCtx<DIR, OUT, NF> cx;
+    cx.wp.clear();
+    cx.wm.clear();
+    cx.fhat_prev = 0.0;
+    cx.alpha = Real<R>::from_bits(a.diag->slot[a.slot].alpha_bits[DIR]);
+    cx.c3 = 39.05;
+    cx.eps = a.eps_eff;
+    cx.coef = a.coef;
+    cx.dt = a.dt;
+    cx.rk_a = a.rk_a;
+    cx.rk_b = a.rk_b;
+    cx.lane = lane;
+    const bool is_energy = (f == 0), is_normal = (f == 1 + DIR);
+    cx.kE = is_energy ? 1.0 : 0.0;
+
+    for (int m = 0; m < nchunks; ++m) {
+        const int cm = s0 - 4 + m * RING_CH;
+        if (m > 0) {
+            fence_proxy_async();                                       // output-tile / fix-up writes -> async proxy
+            if (leader) tma_wait_read0();                              // the write-back issued one chunk ago has read its tile
+            __syncthreads();                                           // everyone is done with chunk m-1
+            if (leader) {
+                if (m > 1) flush(m - 1);
+                if (m + 1 < nchunks) issue(m + 1);                     // overwrites chunk m-2
+            }
+        }
+        R* st = stages + (m % RING_NSTAGE) * STAGE_REALS;
+        const R* stp = stages + ((m + RING_NSTAGE - 1) % RING_NSTAGE) * STAGE_REALS;   // chunk m-1
+        mbar_wait(&full[m % RING_NSTAGE], (m / RING_NSTAGE) & 1);
+
+        // a-7: ghost rows (block-uniform test; at most the first and the last two chunks of a grid line)
+        if (cm < 0 || cm + RING_CH - 1 > nd - 1) {
+            const int rlast = nd - 1 - cm;                             // row of the last interior cell (may be < 0)
+            for (int t = f; t < NF + 2; t += NF) {
+#pragma unroll
+                for (int r = 0; r < RING_CH; ++r) {
+                    const int c = cm + r;
+                    if (c < 0) st[t * RING_SUB + sub_off<DIR>(r, lane)] = st[t * RING_SUB + sub_off<DIR>(-cm, lane)];
+                    else if (c > nd - 1) {
+                        st[t * RING_SUB + sub_off<DIR>(r, lane)] =
+                            rlast >= 0 ? st[t * RING_SUB + sub_off<DIR>(rlast, lane)]
+                                       : stp[t * RING_SUB + sub_off<DIR>(rlast + RING_CH, lane)];
+                    }
+                }
+            }
+            __syncthreads();
+        }
+
+        cx.pu.set(st + f * RING_SUB, lane);
+        cx.pmd.set(st + (1 + DIR) * RING_SUB, lane);
+        cx.pa.set(is_energy ? st + (1 + DIR) * RING_SUB : st + f * RING_SUB, lane);
+        cx.pw.set(is_energy ? zeros : st + NF * RING_SUB, lane);
+        cx.pp.set(is_normal ? st + (NF + 1) * RING_SUB : zeros, lane);
+        if (OUT == OUT_COMBINE1 || OUT == OUT_COMBINE) {
+            cx.pus[0].set(stp + f * RING_SUB, lane);
+            cx.pus[1].set(st + f * RING_SUB, lane);
+        }
+        if (OUT == OUT_COMBINE) cx.pun.set(unt + (m & 1) * NF * RING_SUB + f * RING_SUB, lane);
+        cx.out = outt + (m & 1) * NF * RING_SUB + f * RING_SUB;
+
+        if (m == 0) {
+            // warm-up chunk: cells s0-4 .. s0+3 fill both windows; the last row gives the interface s0 - 1/2
+            cx.template load_push<0>(); cx.template load_push<1>(); cx.template load_push<2>(); cx.template load_push<3>();
+            cx.template load_push<4>(); cx.template load_push<5>(); cx.template load_push<6>(); cx.template load_push<7>();
+            cx.fhat_prev = rot_flux<7>(cx.wp, cx.wm);
+        } else {
+            cx.template row<0>(); cx.template row<1>(); cx.template row<2>(); cx.template row<3>();
+            cx.template row<4>(); cx.template row<5>(); cx.template row<6>(); cx.template row<7>();
+        }
+    }
+    fence_proxy_async();
+    if (leader) tma_wait_read0();
+    __syncthreads();
+    if (leader) {
+        if (nchunks > 1) flush(nchunks - 1);
+        tma_wait_all0();
+    }
+}
+
+}  // namespace hydro_dev
