@@ -42,6 +42,24 @@ UNIT = "cell-updates/s"
 FLOPS_STAGE = {4: 3764.0, 5: 4691.0}
 FLOPS_SWEEPS_STAGE = {4: 3 * (1208.0 + 12.0) + 20.0, 5: 3 * (1510.0 + 15.0) + 25.0}
 FP64_NOMINAL_TF = 148 * 64 * 2 * 1.965e9 / 1e12          # 148 SMs x 64 DFMA/clk x 2 x 1.965 GHz = 37.2
+# dram__bytes_read.sum + dram__bytes_write.sum per sweep launch at 256^3 fp64 nf=4, mean of the x (COMBINE), y and z
+# (REDUCE) kernels, from the one `ncu --set full` capture summarised in profiles/r1_c_ring_ncu_summary.txt
+NCU_TRAFFIC_SWEEP_256_F64_NF4 = (1.310e9 + 1.837e9 + 1.839e9) / 3.0
+
+
+def max_over_ranks(values, world, device):
+    """MAX over ranks of a list of floats (times): the contract's max-over-ranks timing.  world == 1: identity."""
+    import torch
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+def job_value(world, cells, steps, seconds):
+    """Whole-job cell-updates/s of `world` independent replicas ("replicas only")."""
+    return world * cells * steps / seconds
 
 
 class ClockSampler:
@@ -246,13 +264,10 @@ def main():
         nbytes = U0h.numel() * U0h.element_size()
         e2e = (t_e2e, nbytes)
 
-    tmax = torch.tensor([ms, e2e[0] if e2e else 0.0], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_max, e2e_max = tmax.tolist()
+    ms_max, e2e_max = max_over_ranks([ms, e2e[0] if e2e else 0.0], world, "cuda")
 
     if rank == 0:
-        value = world * cells * args.steps / (ms_max * 1e-3)
+        value = job_value(world, cells, args.steps, ms_max * 1e-3)
         nf = c["nf"]
         sweeps = [kt[k] for k in ("sweep_x", "sweep_y", "sweep_z")]
         sw_ms = sum(k["ms"] for k in sweeps)
@@ -262,7 +277,8 @@ def main():
         fl_launch = FLOPS_SWEEPS_STAGE[nf] / 3.0 * cells
         achieved = fl_launch / (sw_ms / sw_n * 1e-3) / 1e12 if sw_n else 0.0
         nominal = FP64_NOMINAL_TF * (1 if args.precision == 64 else 2)
-        roof = {"bound": "alu", "kernel": "k_sweep<x|y|z> (WENO7-LF flux + divergence [+ RK3 combine])",
+        roof = {"bound": "alu", "kernel": "k_sweep_ring<x|y|z> (WENO7-LF flux + divergence + RK3 combine)" if g.uses_ring() else
+                          "k_sweep<x|y|z> (generic path)",
                 "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf,
                 "peak_kind": "measured in this run: register-resident %s chain on all SMs (hydro_measure_alu_peak)" %
                              ("DFMA" if args.precision == 64 else "FFMA"),
@@ -271,7 +287,9 @@ def main():
                 "share_of_step": sw_ms / all_ms if all_ms else None,
                 "kernel_ms_per_step": {k: v["ms"] / args.steps for k, v in kt.items()},
                 "whole_path_frac": (FLOPS_STAGE[nf] * 3 * value) / (peak_tf * 1e12),
-                "traffic": None}
+                "traffic": NCU_TRAFFIC_SWEEP_256_F64_NF4 if (cfg == 3 and args.precision == 64 and g.uses_ring()) else None,
+                "traffic_source": "profiles/r1_c_ring_ncu_summary.txt (ncu --set full, dram read+write per launch)",
+                "algorithmic_bytes_per_launch": (nf + 2 + nf + nf * 2.0 / 9.0 + 2.0 / 3.0 * nf) * 8.0 * cells}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
@@ -281,7 +299,7 @@ def main():
             "diag": {"ncap": dg["ncap"], "alpha": dg["alpha"].tolist(), "deposited_E_GeV": float(dg["deposited"][0])},
         }
         if e2e:
-            line["e2e"] = {"value": world * cells * args.steps / e2e_max, "unit": UNIT,
+            line["e2e"] = {"value": job_value(world, cells, args.steps, e2e_max), "unit": UNIT,
                            "h2d_bytes_per_step": e2e[1] / args.steps, "d2h_bytes_per_step": e2e[1] / args.steps,
                            "what": "hydro_set_state(host) + hydro_step(K) + hydro_get_fields(host), pinned buffers; "
                                    "bytes are the one upload / one download spread over K steps"}

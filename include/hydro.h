@@ -105,6 +105,10 @@ int hydro_get_last_stage_q(hydro_t *h, int jet, double out[3]);
 int hydro_set_profiling(hydro_t *h, int enable);
 int hydro_get_kernel_times(hydro_t *h, double ms[HYDRO_K_COUNT], long long launches[HYDRO_K_COUNT]);
 
+/* Which sweep kernels this handle uses: 1 = TMA ring kernels (fp64 and even nx: hydro_sweep_ring.cuh), 0 = generic
+ * direct-load kernels (fp32, or odd nx where rows are not 16-byte aligned).  Same arithmetic either way. */
+int hydro_sweep_path(const hydro_t *h);
+
 /* Number of kernel launches hydro_step has enqueued on this handle since create. */
 long long hydro_launch_count(const hydro_t *h);
 

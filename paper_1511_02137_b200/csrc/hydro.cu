@@ -219,6 +219,8 @@ int setup_tma(hydro* h) {
         while (blocks1 * seg < (long long)h->num_sms * 3 && nd[d] / (seg * 2) >= 16) seg *= 2;
         int ls = (nd[d] + seg - 1) / seg;
         ls = (ls + RING_CH - 1) / RING_CH * RING_CH;
+        const char* force = getenv("HYDRO_SEG_LEN");                  // tuning knob: march cells per block
+        if (force && atoi(force) >= RING_CH) ls = atoi(force) / RING_CH * RING_CH;
         h->seg_len[d] = ls;
         h->tma_nseg[d] = (nd[d] + ls - 1) / ls;
     }
@@ -580,6 +582,8 @@ int hydro_get_kernel_times(hydro_t* h, double ms[HYDRO_K_COUNT], long long launc
 }
 
 long long hydro_launch_count(const hydro_t* h) { return h ? h->launches : -1; }
+
+int hydro_sweep_path(const hydro_t* h) { return h && h->use_tma ? 1 : 0; }
 
 int hydro_measure_alu_peak(int precision, double millis, void* cuda_stream, double* tflops) {
     if (!tflops || (precision != 64 && precision != 32) || !(millis > 0)) return HYDRO_EINVAL;

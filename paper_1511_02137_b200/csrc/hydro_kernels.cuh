@@ -61,6 +61,27 @@ template <> struct Real<double> {
         r = fma(r, e, r);
         return r;
     }
+    // 1/x and sqrt(x) for normal, positive, well-scaled x without the special-case paths of the IEEE routines
+    // (error <= ~1 ulp): hardware seeds (upper 32 bits, ~2^-20) + Newton-type corrections.
+    static __device__ __forceinline__ double rcp_fast(double x) {
+        double r;
+        asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+        const double e = fma(-x, r, 1.0);
+        r = fma(r, fma(e, e, e), r);                    // cubic step: error e^3
+        return fma(r, fma(-x, r, 1.0), r);              // + one linear step: last-bit accuracy
+    }
+    static __device__ __forceinline__ double sqrt_fast(double x) {
+        double y;
+        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+        double g = x * y, h = 0.5 * y;                  // g ~ sqrt(x), h ~ 1/(2 sqrt(x))
+        double r = fma(-g, h, 0.5);
+        g = fma(g, r, g);
+        h = fma(h, r, h);
+        r = fma(-g, h, 0.5);
+        g = fma(g, r, g);
+        h = fma(h, r, h);
+        return fma(fma(-g, g, x), h, g);                // final residual correction
+    }
 };
 template <> struct Real<float> {
     typedef unsigned int bits_t;
@@ -69,6 +90,8 @@ template <> struct Real<float> {
     static __device__ __forceinline__ float sqrt_(float x) { return sqrtf(x); }
     static __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
     static __device__ __forceinline__ float rcp_(float x) { return 1.0f / x; }
+    static __device__ __forceinline__ float rcp_fast(float x) { return 1.0f / x; }
+    static __device__ __forceinline__ float sqrt_fast(float x) { return sqrtf(x); }
 };
 
 // ------------------------------------------------------------------------------------------------ a-1, a-2
@@ -78,33 +101,36 @@ template <> struct Real<float> {
 template <typename R>
 __device__ __forceinline__ void con2prim(R E, R Mx, R My, R Mz, R e_floor, R one_minus_delta, R& p, R& wt,
                                          int& limited) {
+    typedef Real<R> T;
     limited = 0;
     if (E < e_floor) { E = e_floor; limited = 1; }
-    R M = Real<R>::sqrt_(Mx * Mx + My * My + Mz * Mz);
-    R cap = one_minus_delta * E;
+    R M2 = Mx * Mx + My * My + Mz * Mz;
+    const R cap = one_minus_delta * E;
     R sc = R(1);
-    if (M > cap) { sc = cap / M; limited = 1; }
-    R mx = Mx * sc, my = My * sc, mz = Mz * sc;
-    R M2 = mx * mx + my * my + mz * mz;
-    R s = Real<R>::sqrt_(R(4) * E * E - R(3) * M2);
-    R e = R(3) * (E * E - M2) / (E + s);
-    p = e / R(3);
-    wt = sc / (E + p);
+    if (M2 > cap * cap) {                                            // rare: |M| > (1 - delta) E
+        sc = cap / T::sqrt_(M2);
+        limited = 1;
+        const R mx = Mx * sc, my = My * sc, mz = Mz * sc;
+        M2 = mx * mx + my * my + mz * mz;
+    }
+    const R s = T::sqrt_fast(R(4) * E * E - R(3) * M2);
+    const R e = R(3) * (E * E - M2) * T::rcp_fast(E + s);
+    p = e * R(1.0 / 3.0);
+    wt = sc * T::rcp_fast(E + p);
 }
 
 // max(|lambda_+|, |lambda_-|) of the acoustic eigenvalues along a direction with velocity component vd:
-// lambda = [vd (1-cs2) +- cs sqrt((1-v2)(1 - v2 cs2 - vd^2 (1-cs2)))] / (1 - v2 cs2),  cs2 = 1/3
+// lambda = [vd (1-cs2) +- cs sqrt((1-v2)(1 - v2 cs2 - vd^2 (1-cs2)))] / (1 - v2 cs2),  cs2 = 1/3;
+// root >= 0 and den > 0, so the larger modulus is (|vd| (1-cs2) + root) / den.
 template <typename R>
-__device__ __forceinline__ R max_wavespeed(R vd, R v2, R inv_den, R om_v2) {
+__device__ __forceinline__ R max_wavespeed(R vd, R den, R inv_den, R om_v2) {
     const R cs2 = R(1.0 / 3.0);
-    R rad = om_v2 * (R(1) - v2 * cs2 - vd * vd * (R(1) - cs2));
-    rad = rad < R(0) ? R(0) : rad;
-    R root = R(0.57735026918962576451) * Real<R>::sqrt_(rad);
+    R rad = om_v2 * (den - vd * vd * (R(1) - cs2));
+    rad = rad < R(1e-30) ? R(1e-30) : rad;                           // clamp (R9); keeps the rsqrt seed finite
+    const R root = R(0.57735026918962576451) * Real<R>::sqrt_fast(rad);
     R a = vd * (R(1) - cs2);
-    R lp = (a + root) * inv_den, lm = (a - root) * inv_den;
-    lp = lp < R(0) ? -lp : lp;
-    lm = lm < R(0) ? -lm : lm;
-    return lp > lm ? lp : lm;
+    a = a < R(0) ? -a : a;
+    return (a + root) * inv_den;
 }
 
 template <typename R>
@@ -123,8 +149,7 @@ __global__ void __launch_bounds__(256) k_prim(PrimArgs<R> a) {
     R am[3] = {R(0), R(0), R(0)};
     unsigned int ncap = 0, bad = 0;
     const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < a.N; c += stride) {
-        R E = a.U[c], Mx = a.U[a.N + c], My = a.U[2 * a.N + c], Mz = a.U[3 * a.N + c];
+    auto cell = [&](long long c, R E, R Mx, R My, R Mz) {
         R p, wt;
         int lim;
         con2prim<R>(E, Mx, My, Mz, a.e_floor, a.one_minus_delta, p, wt, lim);
@@ -137,14 +162,26 @@ __global__ void __launch_bounds__(256) k_prim(PrimArgs<R> a) {
         R vx = Mx * wt, vy = My * wt, vz = Mz * wt;
         R v2 = vx * vx + vy * vy + vz * vz;
         R om = R(1) - v2;
-        R inv_den = R(1) / (R(1) - v2 * R(1.0 / 3.0));
-        R lx = max_wavespeed<R>(vx, v2, inv_den, om);
-        R ly = max_wavespeed<R>(vy, v2, inv_den, om);
-        R lz = max_wavespeed<R>(vz, v2, inv_den, om);
+        om = om < R(0) ? R(0) : om;
+        const R den = R(1) - v2 * R(1.0 / 3.0);
+        const R inv_den = Real<R>::rcp_fast(den);
+        R lx = max_wavespeed<R>(vx, den, inv_den, om);
+        R ly = max_wavespeed<R>(vy, den, inv_den, om);
+        R lz = max_wavespeed<R>(vz, den, inv_den, om);
         am[0] = lx > am[0] ? lx : am[0];
         am[1] = ly > am[1] ? ly : am[1];
         am[2] = lz > am[2] ? lz : am[2];
+    };
+    // two cells per trip: eight independent loads in flight per thread before the arithmetic starts
+    long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; c + stride < a.N; c += 2 * stride) {
+        const long long c2 = c + stride;
+        const R E = a.U[c], Mx = a.U[a.N + c], My = a.U[2 * a.N + c], Mz = a.U[3 * a.N + c];
+        const R E2 = a.U[c2], Mx2 = a.U[a.N + c2], My2 = a.U[2 * a.N + c2], Mz2 = a.U[3 * a.N + c2];
+        cell(c, E, Mx, My, Mz);
+        cell(c2, E2, Mx2, My2, Mz2);
     }
+    if (c < a.N) cell(c, a.U[c], a.U[a.N + c], a.U[2 * a.N + c], a.U[3 * a.N + c]);
     // warp reduction by shuffles, then one atomic per warp on the bit pattern (non-negative reals order like
     // unsigned integers; the max is exact, hence order independent)
     unsigned long long ab[3];

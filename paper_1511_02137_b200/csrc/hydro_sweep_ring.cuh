@@ -181,7 +181,7 @@ __device__ __forceinline__ void weno7_diff(double D0, double D1, double D2, doub
     const double a123 = fma(12.0, u1, a23);
     den = u0 + a123;
     num12 = fma(a123, 3.0 * G0, fma(-a23, G1, a3 * G2));
-    base12 = fma(13.0, D2, fma(-10.0, D1, 3.0 * D0));
+    base12 = lam0 + m0;                                   // 3 D_0 - 10 D_1 + 13 D_2 = lam_0 + m_0 identically
 }
 
 // reciprocal of a normal, well-scaled double: hardware seed (the upper 32 bits of the operand and of the result,

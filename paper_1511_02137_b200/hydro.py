@@ -24,7 +24,7 @@ K_NAMES = ("prim", "sweep_x", "sweep_y", "sweep_z", "source")
 # every symbol include/hydro.h declares (tests check that the library exports all of them)
 SYMBOLS = ("hydro_create", "hydro_destroy", "hydro_set_state", "hydro_add_jet", "hydro_clear_jets", "hydro_step",
            "hydro_synchronize", "hydro_get_fields", "hydro_eval_rhs", "hydro_get_diag", "hydro_get_last_stage_q",
-           "hydro_set_profiling", "hydro_get_kernel_times", "hydro_launch_count", "hydro_measure_alu_peak",
+           "hydro_set_profiling", "hydro_get_kernel_times", "hydro_launch_count", "hydro_sweep_path", "hydro_measure_alu_peak",
            "hydro_strerror", "hydro_last_cuda_error")
 
 
@@ -81,6 +81,8 @@ def load():
     L.hydro_get_kernel_times.argtypes = [vp, dp, C.POINTER(ll)]
     L.hydro_launch_count.restype = ll
     L.hydro_launch_count.argtypes = [vp]
+    L.hydro_sweep_path.restype = i
+    L.hydro_sweep_path.argtypes = [vp]
     L.hydro_measure_alu_peak.restype = i
     L.hydro_measure_alu_peak.argtypes = [i, d, vp, dp]
     L.hydro_strerror.restype = C.c_char_p
@@ -229,3 +231,6 @@ class Hydro:
 
     def launch_count(self):
         return self.L.hydro_launch_count(self.h)
+
+    def uses_ring(self):
+        return self.L.hydro_sweep_path(self.h) == 1

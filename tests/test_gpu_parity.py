@@ -233,6 +233,76 @@ def test_config2_midsize(H, oracle):
     g.close(), o.close()
 
 
+def test_config3_full_size_first_steps(H, oracle):
+    """BASELINE config 3 at its full size (256^3), in the launch configuration bench.py times (ring kernels, one
+    segment per line): HYDRO_TEST_CFG3_STEPS (default 2) of its 120 steps against the oracle on every cell (the
+    oracle needs ~4-8 s per step on the box's cores and ~3 GB)."""
+    steps = int(os.environ.get("HYDRO_TEST_CFG3_STEPS", "2"))
+    c, U0, g, o = make_pair(H, oracle, 3)
+    assert g.uses_ring()
+    g.step(steps)
+    o.step(steps)
+    errs = r13(g.get_fields(), o.get_fields())
+    assert max(errs) < TOL_RUN, errs
+    compare_diag(g, o, steps)
+    g.close(), o.close()
+
+
+def test_config3_long_run_properties(H):
+    """Config 3 for its full 120 steps on the GPU alone, in bench.py's launch configuration: properties that hold at
+    any size.  Pin P5 on the device: the run with the jet and the run without it differ in total energy and
+    momentum by exactly the deposited amounts (the jet's wake has not reached the boundary by t = 2.4 fm/c, so the
+    boundary fluxes of the two runs agree up to the tiny change of the global Lax-Friedrichs alpha); the state stays
+    finite; a repeated run is bitwise identical (reduce-adds are ordered by the stream)."""
+    c = S.CONFIGS[3]
+    U0 = S.make_state(3)
+    g = H.Hydro(*c["n"], c["dx"], c["dt"])
+    assert g.uses_ring()
+    g.set_state(U0)
+    g.step(c["steps"])
+    tot0 = [U.sum(dtype=np.longdouble) for U in g.get_fields()]
+    for pos, d in c["jets"]:
+        g.add_jet(pos, d)
+    g.set_state(U0)
+    g.step(c["steps"])
+    U = g.get_fields()
+    dg = g.diag()
+    assert dg["has_nan"] == 0 and dg["step"] == c["steps"] and np.all(np.isfinite(U))
+    dep = dg["deposited"]
+    assert dep[0] > 5.0 and dep[1] == pytest.approx(dep[0], rel=1e-12) and dep[2] == 0.0 and dep[3] == 0.0
+    dx3 = c["dx"] ** 3
+    for f in range(4):
+        diff = float((U[f].sum(dtype=np.longdouble) - tot0[f]) * dx3)
+        assert abs(diff - dep[f]) <= 5e-5 * dep[0], (f, diff, dep[f])      # measured 6e-6 (alpha: 0.97 -> 1.0 with the jet)
+    g.set_state(U0)
+    g.step(c["steps"])
+    assert np.array_equal(g.get_fields(), U)
+    g.close()
+
+
+@pytest.mark.parametrize("cfg,n,steps", [(0, (32, 32, 32), 10), (2, (64, 32, 32), 30), (0, (33, 20, 17), 6)])
+def test_fp32_variant(H, oracle, cfg, n, steps):
+    """fp32 variant (R10): storage and arithmetic in fp32, compared with the fp64 oracle run with delta = 1e-5,
+    north_star tolerance 1e-4 (R13 metric)."""
+    c = S.scaled_config(cfg, n)
+    if cfg == 2:
+        c["jets"] = [((-2.0, 0.0, 0.0), (1.0, 0.0, 0.0))]
+    U0 = S.make_state(c)
+    g = H.Hydro(*c["n"], c["dx"], c["dt"], precision=32)
+    o = oracle.Oracle(*c["n"], c["dx"], c["dt"], v_cap_delta=1e-5)
+    g.set_state(U0.astype(np.float32))
+    o.set_state(U0.astype(np.float32).astype(np.float64))
+    for pos, d in c["jets"]:
+        g.add_jet(pos, d)
+        o.add_jet(pos, d)
+    g.step(steps)
+    o.step(steps)
+    errs = r13(g.get_fields().astype(np.float64), o.get_fields())
+    assert max(errs) < 1e-4, errs
+    assert g.diag()["has_nan"] == 0
+    g.close(), o.close()
+
+
 # ------------------------------------------------------------------------------------------------ invariants on the GPU
 def test_gpu_uniform_state_and_symmetry(H):
     n = (40, 24, 17)
