@@ -123,7 +123,7 @@ int buf_index(const hydro* h, const void* U) {
 
 // One ring sweep (hydro_sweep_ring.cuh).  `Us` must be one of the three state buffers; `out_map` is the tensor map
 // (for direction DIR) of the buffer the result is stored / reduced into; `un_map` that of U^n (OUT_COMBINE).
-template <int DIR, int OUT, int NF>
+template <typename R, int DIR, int OUT, int NF>
 int launch_ring_nf(hydro* h, const void* Us, int slot, const CUtensorMap* out_map, const CUtensorMap* un_map, double coef,
                    double rk_a, double rk_b) {
     const int b = buf_index(h, Us);
@@ -139,29 +139,30 @@ int launch_ring_nf(hydro* h, const void* Us, int slot, const CUtensorMap* out_ma
     dim3 block(32, NF, 1);
     {
         Timer t(h, HYDRO_K_SWEEP_X + DIR);
-        k_sweep_ring<DIR, OUT, NF><<<grid, block, ring_smem_bytes(NF, OUT), h->stream>>>(m, a);
+        k_sweep_ring<R, DIR, OUT, NF><<<grid, block, ring_smem_bytes(NF, OUT, sizeof(R)), h->stream>>>(m, a);
     }
     h->launches += 1;
     CK(cudaGetLastError());
     return HYDRO_OK;
 }
 
-template <int DIR, int OUT>
+template <typename R, int DIR, int OUT>
 int launch_ring(hydro* h, const void* Us, int slot, const CUtensorMap* out_map, const CUtensorMap* un_map, double coef,
                 double rk_a, double rk_b) {
-    return h->nf == 4 ? launch_ring_nf<DIR, OUT, 4>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b)
-                      : launch_ring_nf<DIR, OUT, 5>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b);
+    return h->nf == 4 ? launch_ring_nf<R, DIR, OUT, 4>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b)
+                      : launch_ring_nf<R, DIR, OUT, 5>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b);
 }
 
-template <int DIR, int OUT, int NF>
+template <typename R, int DIR, int OUT, int NF>
 int set_smem_attr() {
-    return cudaFuncSetAttribute(k_sweep_ring<DIR, OUT, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                ring_smem_bytes(NF, OUT)) == cudaSuccess ? 0 : 1;
+    return cudaFuncSetAttribute(k_sweep_ring<R, DIR, OUT, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                ring_smem_bytes(NF, OUT, sizeof(R))) == cudaSuccess ? 0 : 1;
 }
-template <int NF>
+template <typename R, int NF>
 int set_smem_attrs() {
-    return set_smem_attr<0, OUT_STORE, NF>() + set_smem_attr<0, OUT_COMBINE1, NF>() + set_smem_attr<0, OUT_COMBINE, NF>() +
-           set_smem_attr<1, OUT_REDUCE, NF>() + set_smem_attr<2, OUT_REDUCE, NF>();
+    return set_smem_attr<R, 0, OUT_STORE, NF>() + set_smem_attr<R, 0, OUT_COMBINE1, NF>() +
+           set_smem_attr<R, 0, OUT_COMBINE, NF>() + set_smem_attr<R, 1, OUT_REDUCE, NF>() +
+           set_smem_attr<R, 2, OUT_REDUCE, NF>();
 }
 
 // 4-D tensor map (x, y, z, field) of one SoA buffer with `nfb` fields; box given per dimension
@@ -178,11 +179,15 @@ int make_map(hydro* h, CUtensorMap* out, void* base, int nfb, const unsigned box
         encode = (PFN_cuTensorMapEncodeTiled_v12000)fn;
     }
     cuuint64_t gdim[4] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny, (cuuint64_t)h->nz, (cuuint64_t)nfb};
-    cuuint64_t gstr[3] = {(cuuint64_t)h->nx * 8, (cuuint64_t)h->nx * h->ny * 8, (cuuint64_t)h->N * 8};
+    const cuuint64_t es8 = (cuuint64_t)h->esz;
+    cuuint64_t gstr[3] = {(cuuint64_t)h->nx * es8, (cuuint64_t)h->nx * h->ny * es8, (cuuint64_t)h->N * es8};
     cuuint32_t bx[4] = {box[0], box[1], box[2], box[3]};
     cuuint32_t es[4] = {1, 1, 1, 1};
-    CUresult r = encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, gdim, gstr, bx, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                        swizzle64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE,
+    // x sweep boxes (8 cells of x innermost = 64 bytes in fp64, 32 bytes in fp32) are swizzled at their own width
+    const CUtensorMapSwizzle swz = !swizzle64 ? CU_TENSOR_MAP_SWIZZLE_NONE
+                                              : (h->esz == 8 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_32B);
+    CUresult r = encode(out, h->esz == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, gdim,
+                        gstr, bx, es, CU_TENSOR_MAP_INTERLEAVE_NONE, swz,
                         CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         char b[96];
@@ -205,7 +210,9 @@ int setup_tma(hydro* h) {
         if ((rc = make_map(h, &h->mapP[d], h->P, 1, b1, d == 0)) != HYDRO_OK) return rc;
         if ((rc = make_map(h, &h->mapL[d], h->L, h->nf, boxes[d], d == 0)) != HYDRO_OK) return rc;
     }
-    if (h->nf == 4 ? set_smem_attrs<4>() : set_smem_attrs<5>()) {
+    const int bad = h->prec == 64 ? (h->nf == 4 ? set_smem_attrs<double, 4>() : set_smem_attrs<double, 5>())
+                                  : (h->nf == 4 ? set_smem_attrs<float, 4>() : set_smem_attrs<float, 5>());
+    if (bad) {
         h->cuda_err = "cudaFuncSetAttribute(max dynamic shared memory) failed";
         return HYDRO_ECUDA;
     }
@@ -216,7 +223,7 @@ int setup_tma(hydro* h) {
         const long long other = d == 2 ? h->ny : h->nz;
         const long long blocks1 = ((nlane + 31) / 32) * other;
         int seg = 1;
-        while (blocks1 * seg < (long long)h->num_sms * 3 && nd[d] / (seg * 2) >= 16) seg *= 2;
+        while (blocks1 * seg < (long long)h->num_sms * ring_blocks_per_sm(h->nf, (int)h->esz) && nd[d] / (seg * 2) >= 16) seg *= 2;
         int ls = (nd[d] + seg - 1) / seg;
         ls = (ls + RING_CH - 1) / RING_CH * RING_CH;
         const char* force = getenv("HYDRO_SEG_LEN");                  // tuning knob: march cells per block
@@ -272,6 +279,7 @@ int launch_source(hydro* h, int slot, int stage, double stage_c, bool commit, do
 
 // Ring path (fp64, even nx).  With Uout: the x sweep stores U_next = a U^n + b (U_s + dt L_x), the source kernel and
 // the y, z sweeps add b dt S, b dt L_y, b dt L_z to it (the stage update is linear in L).  Without: L into h->L.
+template <typename R>
 int eval_stage_ring(hydro* h, const void* Uin, int slot, int stage, double stage_c, bool commit, double rk_weight,
                     void* Uout, const void* Un, double rk_a, double rk_b) {
     const double hid = 0.5 / h->dx;
@@ -279,25 +287,25 @@ int eval_stage_ring(hydro* h, const void* Uin, int slot, int stage, double stage
     if (Uout) {
         const int bo = buf_index(h, Uout), bn = Un ? buf_index(h, Un) : -1;
         if (bo < 0 || (Un && bn < 0)) return HYDRO_ESTATE;
-        if (Un) rc = launch_ring<0, OUT_COMBINE>(h, Uin, slot, &h->mapU[bo][0], &h->mapU[bn][0], hid, rk_a, rk_b);
-        else rc = launch_ring<0, OUT_COMBINE1>(h, Uin, slot, &h->mapU[bo][0], 0, hid, 0.0, 1.0);
+        if (Un) rc = launch_ring<R, 0, OUT_COMBINE>(h, Uin, slot, &h->mapU[bo][0], &h->mapU[bn][0], hid, rk_a, rk_b);
+        else rc = launch_ring<R, 0, OUT_COMBINE1>(h, Uin, slot, &h->mapU[bo][0], 0, hid, 0.0, 1.0);
         if (rc != HYDRO_OK) return rc;
         const double bdt = (Un ? rk_b : 1.0) * h->dt;
-        if ((rc = launch_source<double>(h, slot, stage, stage_c, commit, rk_weight, Uout, bdt)) != HYDRO_OK) return rc;
-        if ((rc = launch_ring<1, OUT_REDUCE>(h, Uin, slot, &h->mapU[bo][1], 0, bdt * hid, 0.0, 0.0)) != HYDRO_OK) return rc;
-        return launch_ring<2, OUT_REDUCE>(h, Uin, slot, &h->mapU[bo][2], 0, bdt * hid, 0.0, 0.0);
+        if ((rc = launch_source<R>(h, slot, stage, stage_c, commit, rk_weight, Uout, bdt)) != HYDRO_OK) return rc;
+        if ((rc = launch_ring<R, 1, OUT_REDUCE>(h, Uin, slot, &h->mapU[bo][1], 0, bdt * hid, 0.0, 0.0)) != HYDRO_OK) return rc;
+        return launch_ring<R, 2, OUT_REDUCE>(h, Uin, slot, &h->mapU[bo][2], 0, bdt * hid, 0.0, 0.0);
     }
-    if ((rc = launch_ring<0, OUT_STORE>(h, Uin, slot, &h->mapL[0], 0, hid, 0.0, 0.0)) != HYDRO_OK) return rc;
-    if ((rc = launch_source<double>(h, slot, stage, stage_c, commit, rk_weight, h->L, 1.0)) != HYDRO_OK) return rc;
-    if ((rc = launch_ring<1, OUT_REDUCE>(h, Uin, slot, &h->mapL[1], 0, hid, 0.0, 0.0)) != HYDRO_OK) return rc;
-    return launch_ring<2, OUT_REDUCE>(h, Uin, slot, &h->mapL[2], 0, hid, 0.0, 0.0);
+    if ((rc = launch_ring<R, 0, OUT_STORE>(h, Uin, slot, &h->mapL[0], 0, hid, 0.0, 0.0)) != HYDRO_OK) return rc;
+    if ((rc = launch_source<R>(h, slot, stage, stage_c, commit, rk_weight, h->L, 1.0)) != HYDRO_OK) return rc;
+    if ((rc = launch_ring<R, 1, OUT_REDUCE>(h, Uin, slot, &h->mapL[1], 0, hid, 0.0, 0.0)) != HYDRO_OK) return rc;
+    return launch_ring<R, 2, OUT_REDUCE>(h, Uin, slot, &h->mapL[2], 0, hid, 0.0, 0.0);
 }
 
 // L(U_in, t_n + stage_c dt) into h->L; if Uout != 0 the stage combination forms the next stage state.
 template <typename R>
 int eval_stage(hydro* h, const void* Uin, int slot, int stage, double stage_c, bool commit, double rk_weight,
                void* Uout, const void* Un, double rk_a, double rk_b) {
-    if (h->use_tma) return eval_stage_ring(h, Uin, slot, stage, stage_c, commit, rk_weight, Uout, Un, rk_a, rk_b);
+    if (h->use_tma) return eval_stage_ring<R>(h, Uin, slot, stage, stage_c, commit, rk_weight, Uout, Un, rk_a, rk_b);
     SweepArgs<R> a;
     a.U = (const R*)Uin; a.P = (const R*)h->P; a.W = (const R*)h->W; a.L = (R*)h->L;
     a.Un = (const R*)Un; a.Uout = (R*)Uout; a.diag = h->diag; a.slot = slot;
@@ -437,9 +445,10 @@ int hydro_create(hydro_t** out, int nx, int ny, int nz, double dx, double dt, co
             while (threads * seg < (long long)h->num_sms * 1024 && nd[d] / (seg * 2) >= 16) seg *= 2;
             h->nseg[d] = seg;
         }
-        // TMA-staged sweeps need 16-byte global strides (even nx in fp64); HYDRO_NO_TMA=1 forces the direct-load kernels
+        // TMA-staged sweeps need 16-byte global strides (nx even in fp64, a multiple of 4 in fp32);
+        // HYDRO_NO_TMA=1 forces the direct-load kernels
         const char* no_tma = getenv("HYDRO_NO_TMA");
-        h->use_tma = o.precision == 64 && nx % 2 == 0 && !(no_tma && no_tma[0] == '1');
+        h->use_tma = (nx * (int)h->esz) % 16 == 0 && !(no_tma && no_tma[0] == '1');
         if (h->use_tma) rc = setup_tma(h);
     } while (0);
     if (rc != HYDRO_OK) {

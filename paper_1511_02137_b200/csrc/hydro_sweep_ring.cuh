@@ -88,12 +88,16 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 
 // shared-memory plan of one launch (host and device agree through these functions); units: reals
 __host__ __device__ constexpr int ring_stage_reals(int nf) { return (nf + 2) * RING_SUB; }
-__host__ __device__ constexpr int ring_smem_bytes(int nf, int out) {
+__host__ __device__ constexpr int ring_smem_bytes(int nf, int out, int esz) {
     return (RING_NSTAGE * ring_stage_reals(nf)            // input ring
             + 2 * nf * RING_SUB                            // two output tiles
             + (out == OUT_COMBINE ? 2 * nf * RING_SUB : 0) // two U^n tiles
-            + RING_SUB) * 8                                // one tile of zeros
+            + RING_SUB) * esz                              // one tile of zeros
            + 64;                                           // mbarriers
+}
+// resident blocks per SM the kernels are compiled for (registers: 65536 / (32 NF threads x blocks))
+__host__ __device__ constexpr int ring_blocks_per_sm(int nf, int esz) {
+    return esz == 8 ? (nf == 4 ? 3 : 2) : (nf == 4 ? 5 : 4);
 }
 
 struct RingMaps {
@@ -113,12 +117,14 @@ struct RingArgs {
 };
 
 // element offset inside a sub-tile of march row r (0..7) for this lane
-template <int DIR>
+template <int DIR, typename R>
 __device__ __forceinline__ int sub_off(int r, int lane) {
     if (DIR == 0) {
-        // dense box layout (8 cells of x fastest, 32 rows): byte = lane*64 + r*8, TMA 64-byte swizzle:
-        // 16-byte chunk index (bits 4..5) ^= address bits 7..8 = (lane >> 1) & 3
-        return lane * 8 + ((((r >> 1) ^ ((lane >> 1) & 3)) << 1) | (r & 1));
+        // dense box layout (8 cells of x fastest, 32 rows of y):
+        //   fp64: byte = lane*64 + r*8, TMA 64-byte swizzle: 16-byte chunk index (bits 4..5) ^= address bits 7..8
+        //   fp32: byte = lane*32 + r*4, TMA 32-byte swizzle: 16-byte chunk index (bit 4)     ^= address bit 7
+        if (sizeof(R) == 8) return lane * 8 + ((((r >> 1) ^ ((lane >> 1) & 3)) << 1) | (r & 1));
+        return lane * 8 + ((((r >> 2) ^ ((lane >> 2) & 1)) << 2) | (r & 3));
     }
     return r * 32 + lane;
 }
@@ -127,61 +133,28 @@ __device__ __forceinline__ int sub_off(int r, int lane) {
 // Undivided differences of one split flux along the march, slot = march row mod 8:
 //   V = value, D = V - V_prev, E = D - D_prev, T = E - E_prev (only the newest is kept), G = T - T_prev,
 //   S = C3 T^2 + eps.  Live at any time: 4 V, 6 D, 5 E, 4 S, 3 G, 1 T (the other slots are dead registers).
+template <typename R>
 struct RotWin {
-    double V[8], D[8], E[8], S[8], G[8], T;
+    R V[8], D[8], E[8], S[8], G[8], T;
     __device__ __forceinline__ void clear() {
 #pragma unroll
-        for (int j = 0; j < 8; ++j) { V[j] = 0.0; D[j] = 0.0; E[j] = 0.0; S[j] = 0.0; G[j] = 0.0; }
-        T = 0.0;
+        for (int j = 0; j < 8; ++j) { V[j] = R(0); D[j] = R(0); E[j] = R(0); S[j] = R(0); G[j] = R(0); }
+        T = R(0);
     }
 };
 
-template <int r>
-__device__ __forceinline__ void rot_push(RotWin& w, double x, double c3, double eps) {
+template <int r, typename R>
+__device__ __forceinline__ void rot_push(RotWin<R>& w, R x, R c3, R eps) {
     constexpr int p = (r + 7) & 7;
-    const double dn = x - w.V[p];
-    const double en = dn - w.D[p];
-    const double tn = en - w.E[p];
+    const R dn = x - w.V[p];
+    const R en = dn - w.D[p];
+    const R tn = en - w.E[p];
     w.G[r] = tn - w.T;
-    w.S[r] = fma(c3 * tn, tn, eps);
+    w.S[r] = Real<R>::fma_(c3 * tn, tn, eps);
     w.V[r] = x;
     w.D[r] = dn;
     w.E[r] = en;
     w.T = tn;
-}
-
-// One WENO7-JS reconstruction (r = 4) from the 1st..4th undivided differences in stencil order (D_j, E_j, G_j) and
-// S_j = 39.05 T_j^2 + eps (formulas: DESIGN.md "WENO7 in difference form"):
-//   candidates   12 (q_0 - x_c) = 3 D_0 - 10 D_1 + 13 D_2,  12 (q_1-q_0) = 3 G_0,  12 (q_2-q_1) = -G_1,  12 (q_3-q_2) = G_2
-//   smoothness   36 beta_k + eps = lam_k^2 + 39 m_k^2 + S_k,
-//                lam_0 = 2 D_0 - 7 D_1 + 11 D_2, lam_1 = lam_0 + 2 G_0, lam_2 = lam_1 - G_1, lam_3 = lam_2 + 2 G_2,
-//                m_0 = 2 E_1 - E_0,  m_1 = m_2 = E_2,  m_3 = 2 E_3 - E_4
-//   weights      omega_k ~ d_k prod_{j != k} (eps + beta_j)^2,  d = (1, 12, 18, 4)/35  (common denominator; range-safe
-//                in fp64)
-// Returns base12 = 12 (q_0 - x_c) and num12/den = 12 sum_k omega_k (q_k - q_0):  W = x_c + (base12 + num12/den)/12.
-__device__ __forceinline__ void weno7_diff(double D0, double D1, double D2, double E0, double E1, double E2, double E3,
-                                           double E4, double S0, double S1, double S2, double S3, double G0, double G1,
-                                           double G2, double& base12, double& num12, double& den) {
-    const double lam0 = fma(11.0, D2, fma(-7.0, D1, 2.0 * D0));
-    const double lam1 = fma(2.0, G0, lam0);
-    const double lam2 = lam1 - G1;
-    const double lam3 = fma(2.0, G2, lam2);
-    const double m0 = fma(2.0, E1, -E0);
-    const double m3 = fma(2.0, E3, -E4);
-    const double e39 = 39.0 * E2;
-    const double b0 = fma(lam0, lam0, fma(39.0 * m0, m0, S0));
-    const double b1 = fma(lam1, lam1, fma(e39, E2, S1));
-    const double b2 = fma(lam2, lam2, fma(e39, E2, S2));
-    const double b3 = fma(lam3, lam3, fma(39.0 * m3, m3, S3));
-    const double t0 = b0 * b0, t1 = b1 * b1, t2 = b2 * b2, t3 = b3 * b3;
-    const double p01 = t0 * t1, p23 = t2 * t3;
-    const double u0 = t1 * p23, u1 = t0 * p23, u2 = t3 * p01, u3 = t2 * p01;
-    const double a3 = 4.0 * u3;
-    const double a23 = fma(18.0, u2, a3);
-    const double a123 = fma(12.0, u1, a23);
-    den = u0 + a123;
-    num12 = fma(a123, 3.0 * G0, fma(-a23, G1, a3 * G2));
-    base12 = lam0 + m0;                                   // 3 D_0 - 10 D_1 + 13 D_2 = lam_0 + m_0 identically
 }
 
 // reciprocal of a normal, well-scaled double: hardware seed (the upper 32 bits of the operand and of the result,
@@ -193,54 +166,104 @@ __device__ __forceinline__ double rcp_cubic(double x) {
     const double t = fma(e, e, e);
     return fma(r, t, r);
 }
+__device__ __forceinline__ float rcp_ulp(float x) {      // MUFU.RCP: 1 ulp, enough for the fp32 variant (R10)
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+// One WENO7-JS reconstruction (r = 4) from the 1st..4th undivided differences in stencil order (D_j, E_j, G_j) and
+// S_j = 39.05 T_j^2 + eps (formulas: DESIGN.md "WENO7 in difference form"):
+//   candidates   12 (q_0 - x_c) = 3 D_0 - 10 D_1 + 13 D_2,  12 (q_1-q_0) = 3 G_0,  12 (q_2-q_1) = -G_1,  12 (q_3-q_2) = G_2
+//   smoothness   36 beta_k + eps = lam_k^2 + 39 m_k^2 + S_k,
+//                lam_0 = 2 D_0 - 7 D_1 + 11 D_2, lam_1 = lam_0 + 2 G_0, lam_2 = lam_1 - G_1, lam_3 = lam_2 + 2 G_2,
+//                m_0 = 2 E_1 - E_0,  m_1 = m_2 = E_2,  m_3 = 2 E_3 - E_4
+//   weights      fp64: omega_k ~ d_k prod_{j != k} (eps + beta_j)^2,  d = (1, 12, 18, 4)/35  (common denominator;
+//                range-safe in fp64);  fp32: omega_k ~ d_k (1/(eps + beta_k))^2, one reciprocal each (R10)
+// Returns base12 = 12 (q_0 - x_c) and num12/den = 12 sum_k omega_k (q_k - q_0):  W = x_c + (base12 + num12/den)/12.
+template <typename R>
+__device__ __forceinline__ void weno7_diff(R D0, R D1, R D2, R E0, R E1, R E2, R E3, R E4, R S0, R S1, R S2, R S3,
+                                           R G0, R G1, R G2, R& base12, R& num12, R& den) {
+    typedef Real<R> T;
+    const R lam0 = T::fma_(R(11), D2, T::fma_(R(-7), D1, R(2) * D0));
+    const R lam1 = T::fma_(R(2), G0, lam0);
+    const R lam2 = lam1 - G1;
+    const R lam3 = T::fma_(R(2), G2, lam2);
+    const R m0 = T::fma_(R(2), E1, -E0);
+    const R m3 = T::fma_(R(2), E3, -E4);
+    const R e39 = R(39) * E2;
+    const R b0 = T::fma_(lam0, lam0, T::fma_(R(39) * m0, m0, S0));
+    const R b1 = T::fma_(lam1, lam1, T::fma_(e39, E2, S1));
+    const R b2 = T::fma_(lam2, lam2, T::fma_(e39, E2, S2));
+    const R b3 = T::fma_(lam3, lam3, T::fma_(R(39) * m3, m3, S3));
+    R u0, u1, u2, u3;
+    if (sizeof(R) == 8) {
+        const R t0 = b0 * b0, t1 = b1 * b1, t2 = b2 * b2, t3 = b3 * b3;
+        const R p01 = t0 * t1, p23 = t2 * t3;
+        u0 = t1 * p23; u1 = t0 * p23; u2 = t3 * p01; u3 = t2 * p01;
+    } else {
+        const float r0 = rcp_ulp((float)b0), r1 = rcp_ulp((float)b1), r2 = rcp_ulp((float)b2), r3 = rcp_ulp((float)b3);
+        u0 = r0 * r0; u1 = r1 * r1; u2 = r2 * r2; u3 = r3 * r3;
+    }
+    const R a3 = R(4) * u3;
+    const R a23 = T::fma_(R(18), u2, a3);
+    const R a123 = T::fma_(R(12), u1, a23);
+    den = u0 + a123;
+    num12 = T::fma_(a123, R(3) * G0, T::fma_(-a23, G1, a3 * G2));
+    base12 = lam0 + m0;                                   // 3 D_0 - 10 D_1 + 13 D_2 = lam_0 + m_0 identically
+}
 
 // 2 F_hat at the interface whose newest needed cell sits in slot r of both windows (plus side lags one slot):
 //   plus  side: cells i-3..i+3 = slots r-7..r-1, centre i   = V[r-4]
 //   minus side: cells i-2..i+4 = slots r-6..r,   centre i+1 = V[r-3], stencil order reversed (D_j = -d[5-j], ...)
-template <int r>
-__device__ __forceinline__ double rot_flux(const RotWin& wp, const RotWin& wm) {
+template <int r, typename R>
+__device__ __forceinline__ R rot_flux(const RotWin<R>& wp, const RotWin<R>& wm) {
 #define SL(k) (((r) + (k) + 16) & 7)
-    double bp, np_, dp, bm, nm, dm;
-    weno7_diff(wp.D[SL(-6)], wp.D[SL(-5)], wp.D[SL(-4)],
-               wp.E[SL(-5)], wp.E[SL(-4)], wp.E[SL(-3)], wp.E[SL(-2)], wp.E[SL(-1)],
-               wp.S[SL(-4)], wp.S[SL(-3)], wp.S[SL(-2)], wp.S[SL(-1)],
-               wp.G[SL(-3)], wp.G[SL(-2)], wp.G[SL(-1)], bp, np_, dp);
-    weno7_diff(-wm.D[SL(0)], -wm.D[SL(-1)], -wm.D[SL(-2)],
-               wm.E[SL(0)], wm.E[SL(-1)], wm.E[SL(-2)], wm.E[SL(-3)], wm.E[SL(-4)],
-               wm.S[SL(0)], wm.S[SL(-1)], wm.S[SL(-2)], wm.S[SL(-3)],
-               wm.G[SL(0)], wm.G[SL(-1)], wm.G[SL(-2)], bm, nm, dm);
-    const double x = fma(np_, dm, nm * dp) * rcp_cubic(dp * dm);
-    return fma((bp + bm) + x, 1.0 / 12.0, wp.V[SL(-4)] + wm.V[SL(-3)]);
+    R bp, np_, dp, bm, nm, dm;
+    weno7_diff<R>(wp.D[SL(-6)], wp.D[SL(-5)], wp.D[SL(-4)],
+                  wp.E[SL(-5)], wp.E[SL(-4)], wp.E[SL(-3)], wp.E[SL(-2)], wp.E[SL(-1)],
+                  wp.S[SL(-4)], wp.S[SL(-3)], wp.S[SL(-2)], wp.S[SL(-1)],
+                  wp.G[SL(-3)], wp.G[SL(-2)], wp.G[SL(-1)], bp, np_, dp);
+    weno7_diff<R>(-wm.D[SL(0)], -wm.D[SL(-1)], -wm.D[SL(-2)],
+                  wm.E[SL(0)], wm.E[SL(-1)], wm.E[SL(-2)], wm.E[SL(-3)], wm.E[SL(-4)],
+                  wm.S[SL(0)], wm.S[SL(-1)], wm.S[SL(-2)], wm.S[SL(-3)],
+                  wm.G[SL(0)], wm.G[SL(-1)], wm.G[SL(-2)], bm, nm, dm);
+    R x;
+    if (sizeof(R) == 8) x = (R)(fma((double)np_, (double)dm, (double)nm * (double)dp) * rcp_cubic((double)dp * (double)dm));
+    else x = (R)fmaf((float)np_, rcp_ulp((float)dp), (float)nm * rcp_ulp((float)dm));
+    return Real<R>::fma_((bp + bm) + x, R(1.0 / 12.0), wp.V[SL(-4)] + wm.V[SL(-3)]);
 #undef SL
 }
 
-// per-thread view of one input stage: byte-free element pointers with the lane offset folded in
-template <int DIR>
+// per-thread view of one input stage: element pointers with the lane offset folded in
+template <int DIR, typename R>
 struct RowPtr {
-    const double* q[DIR == 0 ? 4 : 1];     // DIR 0: one pointer per swizzle class (r >> 1)
-    __device__ __forceinline__ void set(const double* tile, int lane) {
+    static constexpr int NCLS = DIR == 0 ? (sizeof(R) == 8 ? 4 : 2) : 1;      // DIR 0: one pointer per swizzle class
+    const R* q[NCLS];
+    __device__ __forceinline__ void set(const R* tile, int lane) {
         if (DIR == 0) {
 #pragma unroll
-            for (int k = 0; k < 4; ++k) q[k] = tile + lane * 8 + ((k ^ ((lane >> 1) & 3)) << 1);
+            for (int k = 0; k < NCLS; ++k)
+                q[k] = tile + lane * 8 + (sizeof(R) == 8 ? ((k ^ ((lane >> 1) & 3)) << 1) : ((k ^ ((lane >> 2) & 1)) << 2));
         } else q[0] = tile + lane;
     }
     template <int r>
-    __device__ __forceinline__ double at() const {
-        if (DIR == 0) return q[r >> 1][r & 1];
+    __device__ __forceinline__ R at() const {
+        if (DIR == 0) return sizeof(R) == 8 ? q[(r >> 1) % NCLS][r & 1] : q[(r >> 2) % NCLS][r & 3];
         return q[0][r * 32];
     }
 };
 
-template <int DIR, int OUT, int NF>
+template <typename R, int DIR, int OUT, int NF>
 struct SweepCtx {
-    RotWin wp, wm;
-    double fhat_prev;
-    double alpha, c3, eps, coef, dt, rk_a, rk_b, kE;
+    RotWin<R> wp, wm;
+    R fhat_prev;
+    R alpha, c3, eps, coef, dt, rk_a, rk_b, kE;
     // current chunk
-    RowPtr<DIR> pu, pmd, pa, pw, pp;       // own field, normal momentum, A operand, W (or zeros), P (or zeros)
-    RowPtr<DIR> pus[2];                    // U_s of the output cells: rows 4..7 of the previous chunk, 0..3 of this one
-    RowPtr<DIR> pun;                       // U^n of the output cells
-    double* out;                           // this field's output sub-tile, lane offset NOT folded in
+    RowPtr<DIR, R> pu, pmd, pa, pw, pp;    // own field, normal momentum, A operand, W (or zeros), P (or zeros)
+    RowPtr<DIR, R> pus[2];                 // U_s of the output cells: rows 4..7 of the previous chunk, 0..3 of this one
+    RowPtr<DIR, R> pun;                    // U^n of the output cells
+    R* out;                                // this field's output sub-tile, lane offset NOT folded in
     int lane;
 
     // split fluxes of the row's cell, carried as 2 f^+- = F +- alpha U:
@@ -249,27 +272,29 @@ struct SweepCtx {
     // momenta / N_B: A = U_f, B = M_d W, C = p (normal component) or 0.
     template <int r>
     __device__ __forceinline__ void load_push() {
-        const double u = pu.template at<r>();
-        const double md = pmd.template at<r>();
-        const double B = fma(md, pw.template at<r>(), kE);
-        const double F = fma(pa.template at<r>(), B, pp.template at<r>());
-        rot_push<r>(wp, fma(alpha, u, F), c3, eps);
-        rot_push<r>(wm, fma(-alpha, u, F), c3, eps);
+        typedef Real<R> T;
+        const R u = pu.template at<r>();
+        const R md = pmd.template at<r>();
+        const R B = T::fma_(md, pw.template at<r>(), kE);
+        const R F = T::fma_(pa.template at<r>(), B, pp.template at<r>());
+        rot_push<r, R>(wp, T::fma_(alpha, u, F), c3, eps);
+        rot_push<r, R>(wm, T::fma_(-alpha, u, F), c3, eps);
     }
     template <int r>
     __device__ __forceinline__ void emit() {
-        const double fhat = rot_flux<r>(wp, wm);
-        const double mdiv = (fhat_prev - fhat) * coef;
+        typedef Real<R> T;
+        const R fhat = rot_flux<r, R>(wp, wm);
+        const R mdiv = (fhat_prev - fhat) * coef;
         fhat_prev = fhat;
-        double o;
+        R o;
         if (OUT == OUT_STORE || OUT == OUT_REDUCE) o = mdiv;
         else {
             // output cell i = (row's cell) - 4: U_s from the ring, row (r + 4) & 7 of the previous / this chunk
-            const double us = pus[r < 4 ? 0 : 1].template at<(r + 4) & 7>();
-            o = fma(dt, mdiv, us);
-            if (OUT == OUT_COMBINE) o = fma(rk_b, o, rk_a * pun.template at<r>());
+            const R us = pus[r < 4 ? 0 : 1].template at<(r + 4) & 7>();
+            o = T::fma_(dt, mdiv, us);
+            if (OUT == OUT_COMBINE) o = T::fma_(rk_b, o, rk_a * pun.template at<r>());
         }
-        out[sub_off<DIR>(r, lane)] = o;
+        out[sub_off<DIR, R>(r, lane)] = o;
     }
     template <int r>
     __device__ __forceinline__ void row() {
@@ -278,10 +303,9 @@ struct SweepCtx {
     }
 };
 
-template <int DIR, int OUT, int NF>
-__global__ void __launch_bounds__(32 * NF, NF == 4 ? 3 : 2)
+template <typename R, int DIR, int OUT, int NF>
+__global__ void __launch_bounds__(32 * NF, ring_blocks_per_sm(NF, sizeof(R)))
 k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
-    typedef double R;
     // 1024-byte alignment: the swizzle pattern is a function of the absolute shared address
     extern __shared__ __align__(1024) unsigned char smem[];
     constexpr int STAGE_REALS = ring_stage_reals(NF);
@@ -316,7 +340,7 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
         for (int s = 0; s < RING_NSTAGE; ++s) mbar_init(&full[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    for (int i = f * 32 + lane; i < RING_SUB; i += 32 * NF) zeros[i] = 0.0;
+    for (int i = f * 32 + lane; i < RING_SUB; i += 32 * NF) zeros[i] = R(0);
     __syncthreads();
 
     auto coords = [&](int cm, int& c0, int& c1, int& c2) {
@@ -352,20 +376,20 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
         if (nchunks > 1) issue(1);
     }
 
-    SweepCtx<DIR, OUT, NF> cx;
+    SweepCtx<R, DIR, OUT, NF> cx;
     cx.wp.clear();
     cx.wm.clear();
-    cx.fhat_prev = 0.0;
+    cx.fhat_prev = R(0);
     cx.alpha = Real<R>::from_bits(a.diag->slot[a.slot].alpha_bits[DIR]);
-    cx.c3 = 39.05;
-    cx.eps = a.eps_eff;
-    cx.coef = a.coef;
-    cx.dt = a.dt;
-    cx.rk_a = a.rk_a;
-    cx.rk_b = a.rk_b;
+    cx.c3 = R(39.05);
+    cx.eps = (R)a.eps_eff;
+    cx.coef = (R)a.coef;
+    cx.dt = (R)a.dt;
+    cx.rk_a = (R)a.rk_a;
+    cx.rk_b = (R)a.rk_b;
     cx.lane = lane;
     const bool is_energy = (f == 0), is_normal = (f == 1 + DIR);
-    cx.kE = is_energy ? 1.0 : 0.0;
+    cx.kE = is_energy ? R(1) : R(0);
 
     for (int m = 0; m < nchunks; ++m) {
         const int cm = s0 - 4 + m * RING_CH;
@@ -389,11 +413,11 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
 #pragma unroll
                 for (int r = 0; r < RING_CH; ++r) {
                     const int c = cm + r;
-                    if (c < 0) st[t * RING_SUB + sub_off<DIR>(r, lane)] = st[t * RING_SUB + sub_off<DIR>(-cm, lane)];
+                    if (c < 0) st[t * RING_SUB + sub_off<DIR, R>(r, lane)] = st[t * RING_SUB + sub_off<DIR, R>(-cm, lane)];
                     else if (c > nd - 1) {
-                        st[t * RING_SUB + sub_off<DIR>(r, lane)] =
-                            rlast >= 0 ? st[t * RING_SUB + sub_off<DIR>(rlast, lane)]
-                                       : stp[t * RING_SUB + sub_off<DIR>(rlast + RING_CH, lane)];
+                        st[t * RING_SUB + sub_off<DIR, R>(r, lane)] =
+                            rlast >= 0 ? st[t * RING_SUB + sub_off<DIR, R>(rlast, lane)]
+                                       : stp[t * RING_SUB + sub_off<DIR, R>(rlast + RING_CH, lane)];
                     }
                 }
             }
@@ -416,7 +440,7 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
             // warm-up chunk: cells s0-4 .. s0+3 fill both windows; the last row gives the interface s0 - 1/2
             cx.template load_push<0>(); cx.template load_push<1>(); cx.template load_push<2>(); cx.template load_push<3>();
             cx.template load_push<4>(); cx.template load_push<5>(); cx.template load_push<6>(); cx.template load_push<7>();
-            cx.fhat_prev = rot_flux<7>(cx.wp, cx.wm);
+            cx.fhat_prev = rot_flux<7, R>(cx.wp, cx.wm);
         } else {
             cx.template row<0>(); cx.template row<1>(); cx.template row<2>(); cx.template row<3>();
             cx.template row<4>(); cx.template row<5>(); cx.template row<6>(); cx.template row<7>();

@@ -280,7 +280,33 @@ def test_config3_long_run_properties(H):
     g.close()
 
 
-@pytest.mark.parametrize("cfg,n,steps", [(0, (32, 32, 32), 10), (2, (64, 32, 32), 30), (0, (33, 20, 17), 6)])
+@pytest.mark.parametrize("n", [(32, 32, 32), (36, 19, 23), (8, 5, 3), (132, 9, 6), (33, 20, 17), (64, 40, 72)])
+@pytest.mark.parametrize("nf", [4, 5])
+def test_fp32_rhs_single_stage(H, oracle, n, nf):
+    """fp32 variant, one evaluation of L(U): ring kernels when nx % 4 == 0, generic kernels otherwise (R10)."""
+    c = S.scaled_config(0, n)
+    c["nf"] = nf
+    c["jets"] = [((-0.12, 0.03, 0.0), (1.0, 0.5, -0.25))]
+    U0 = S.make_state(c).astype(np.float32)
+    g = H.Hydro(*n, c["dx"], c["dt"], nfields=nf, precision=32)
+    o = oracle.Oracle(*n, c["dx"], c["dt"], nfields=nf, v_cap_delta=1e-5)
+    assert g.uses_ring() == (n[0] % 4 == 0)
+    g.set_state(U0)
+    o.set_state(U0.astype(np.float64))
+    for pos, d in c["jets"]:
+        g.add_jet(pos, d)
+        o.add_jet(pos, d)
+    for stage_c in (0.0, 0.5):
+        Lg, Lo = g.eval_rhs(stage_c).astype(np.float64), o.eval_rhs(stage_c)
+        scale = np.max(np.abs(Lo), axis=(1, 2, 3))
+        for f in range(nf):
+            assert np.max(np.abs(Lg[f] - Lo[f])) <= 1e-4 * max(scale[f], scale[0]), (f, stage_c)
+        assert np.max(np.abs(g.diag()["alpha"] - o.diag()["alpha"])) < 1e-5
+    g.close(), o.close()
+
+
+@pytest.mark.parametrize("cfg,n,steps", [(0, (32, 32, 32), 10), (2, (64, 32, 32), 30), (0, (33, 20, 17), 6),
+                                         (0, (44, 27, 18), 6)])
 def test_fp32_variant(H, oracle, cfg, n, steps):
     """fp32 variant (R10): storage and arithmetic in fp32, compared with the fp64 oracle run with delta = 1e-5,
     north_star tolerance 1e-4 (R13 metric)."""
