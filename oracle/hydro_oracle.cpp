@@ -177,6 +177,37 @@ void weno7_beta_sos(double a, double b, double c, double d, double e, double f, 
     beta[3] = L1 * L1 / 576.0 + 13.0 / 12.0 * L2 * L2 + 781.0 / 720.0 * L3 * L3;
 }
 
+// ---------------------------------------------------------------- WENO5 (r = 3), WENO-JS  [SURVEY 8(f) f-2]
+// the authors also implemented the 5th-order WENO.  Value at the right face i+1/2 of the centre
+// cell `c` from a..e = phi_{i-2}..phi_{i+2}: three quadratic candidates with the prescribed cell averages,
+// ideal weights (1, 6, 3)/10, smoothness indicators from the integral definition
+// beta_k = sum_{l=1}^{2} int_cell dx^{2l-1} (d^l p_k/dx^l)^2 dx, same nonlinear weights as O5 (R3).
+template <class R>
+void weno5_parts(R a, R b, R c, R d, R e, R q[3], R beta[3]) {
+    q[0] = (R(2.0) * a - R(7.0) * b + R(11.0) * c) / R(6.0);
+    q[1] = (-b + R(5.0) * c + R(2.0) * d) / R(6.0);
+    q[2] = (R(2.0) * c + R(5.0) * d - e) / R(6.0);
+    R s0 = a - R(2.0) * b + c, l0 = a - R(4.0) * b + R(3.0) * c;
+    R s1 = b - R(2.0) * c + d, l1 = b - d;
+    R s2 = c - R(2.0) * d + e, l2 = R(3.0) * c - R(4.0) * d + e;
+    beta[0] = R(13.0 / 12.0) * s0 * s0 + R(0.25) * l0 * l0;
+    beta[1] = R(13.0 / 12.0) * s1 * s1 + R(0.25) * l1 * l1;
+    beta[2] = R(13.0 / 12.0) * s2 * s2 + R(0.25) * l2 * l2;
+}
+const double WENO5_D[3] = {0.1, 0.6, 0.3};
+template <class R>
+R weno5(R a, R b, R c, R d, R e, double eps) {
+    R q[3], beta[3], al[3];
+    weno5_parts(a, b, c, d, e, q, beta);
+    for (int k = 0; k < 3; ++k) {
+        R t = R(eps) + beta[k];
+        al[k] = R(WENO5_D[k]) / (t * t);
+    }
+    R sum = al[0] + al[1] + al[2];
+    R num = al[0] * q[0] + al[1] * q[1] + al[2] * q[2];
+    return num / sum;
+}
+
 // ---------------------------------------------------------------- a-3: physical flux along d
 // F^d = (M_d, M_x v_d + p delta_xd, M_y v_d + p delta_yd, M_z v_d + p delta_zd [, N_B v_d])
 template <class R>
@@ -193,7 +224,7 @@ void phys_flux(int d, const R U[5], const Prim<R>& P, int nf, R F[5]) {
 // NOTE reading R9: fluxes use the *limited* momenta consistently?  No: O3 says only the
 // primitives are limited; U entering F^d_E = M_d and the alpha*U term is the stored U.
 template <class R>
-void interface_flux(int d, int nf, const R Uw[8][5], const Prim<R> Pw[8], R alpha, double eps, R Fhat[5]) {
+void interface_flux(int d, int nf, const R Uw[8][5], const Prim<R> Pw[8], R alpha, double eps, R Fhat[5], int order = 7) {
     R fp[8][5], fm[8][5];
     for (int m = 0; m < 8; ++m) {
         R F[5];
@@ -204,8 +235,14 @@ void interface_flux(int d, int nf, const R Uw[8][5], const Prim<R> Pw[8], R alph
         }
     }
     for (int q = 0; q < nf; ++q) {
-        R wp = weno7(fp[0][q], fp[1][q], fp[2][q], fp[3][q], fp[4][q], fp[5][q], fp[6][q], eps);
-        R wm = weno7(fm[7][q], fm[6][q], fm[5][q], fm[4][q], fm[3][q], fm[2][q], fm[1][q], eps);
+        R wp, wm;
+        if (order == 5) {            // cells i-2..i+2 for f+, i+3..i-1 (mirrored) for f-   [f-2]
+            wp = weno5(fp[1][q], fp[2][q], fp[3][q], fp[4][q], fp[5][q], eps);
+            wm = weno5(fm[6][q], fm[5][q], fm[4][q], fm[3][q], fm[2][q], eps);
+        } else {
+            wp = weno7(fp[0][q], fp[1][q], fp[2][q], fp[3][q], fp[4][q], fp[5][q], fp[6][q], eps);
+            wm = weno7(fm[7][q], fm[6][q], fm[5][q], fm[4][q], fm[3][q], fm[2][q], fm[1][q], eps);
+        }
         Fhat[q] = wp + wm;
     }
 }
@@ -229,7 +266,7 @@ int jet_axis_index(double x, int n, double dx) {
 }
 
 struct Oracle {
-    int nx, ny, nz, nf;
+    int nx, ny, nz, nf, order;      // order: 7 (the paper's scheme) or 5 (its WENO5 variant, f-2)
     double dx, dt, eps, delta, e_floor;
     long long step;                 // integer step counter; t = step*dt (O1)
     std::vector<double> U, U1, U2, L;
@@ -304,7 +341,7 @@ void eval_rhs(Oracle& o, const std::vector<double>& U, double stage_c, std::vect
                         for (int q = 0; q < nf; ++q) Uw[m][q] = U[q * N + c];
                         Pw[m] = o.P[c];
                     }
-                    interface_flux<double>(d, nf, Uw, Pw, alpha, o.eps, &Fh[(size_t)(i + 1) * 5]);
+                    interface_flux<double>(d, nf, Uw, Pw, alpha, o.eps, &Fh[(size_t)(i + 1) * 5], o.order);
                 }
                 for (int i = 0; i < nd; ++i) {
                     size_t c = d == 0 ? o.idx(i, ta, tb) : d == 1 ? o.idx(ta, i, tb) : o.idx(ta, tb, i);
@@ -370,7 +407,7 @@ void* oracle_create(int nx, int ny, int nz, double dx, double dt, int nfields, d
     Oracle* o = new Oracle();
     o->nx = nx; o->ny = ny; o->nz = nz; o->nf = nfields; o->dx = dx; o->dt = dt;
     o->eps = weno_eps; o->delta = v_cap_delta; o->e_floor = e_floor;
-    o->step = 0; o->ncap = 0; o->has_nan = 0;
+    o->step = 0; o->ncap = 0; o->has_nan = 0; o->order = 7;
     size_t T = o->N() * nfields;
     o->U.assign(T, 0.0); o->U1.assign(T, 0.0); o->U2.assign(T, 0.0); o->L.assign(T, 0.0);
     o->P.resize(o->N());
@@ -380,6 +417,12 @@ void* oracle_create(int nx, int ny, int nz, double dx, double dt, int nfields, d
     return o;
 }
 void oracle_destroy(void* h) { delete (Oracle*)h; }
+// spatial order of the reconstruction: 7 (default, "currently we use") or 5 (f-2); returns 0 on success
+int oracle_set_weno_order(void* h, int order) {
+    if (order != 5 && order != 7) return 1;
+    ((Oracle*)h)->order = order;
+    return 0;
+}
 
 // U: nfields blocks of nz*ny*nx doubles, x fastest.  Resets step counter; keeps jets.
 void oracle_set_state(void* h, const double* U) {
@@ -458,7 +501,26 @@ void oracle_weno7_parts(const double v[7], double eps, double q[4], double beta[
     for (int k = 0; k < 4; ++k) { double t = eps + beta[k]; al[k] = WENO_D[k] / (t * t); s += al[k]; }
     for (int k = 0; k < 4; ++k) omega[k] = al[k] / s;
 }
+double oracle_weno5(const double v[5], double eps) { return weno5<double>(v[0], v[1], v[2], v[3], v[4], eps); }
+// q[3] candidates, beta[3], omega[3] nonlinear weights of the r = 3 scheme
+void oracle_weno5_parts(const double v[5], double eps, double q[3], double beta[3], double omega[3]) {
+    weno5_parts<double>(v[0], v[1], v[2], v[3], v[4], q, beta);
+    double al[3], s = 0;
+    for (int k = 0; k < 3; ++k) { double t = eps + beta[k]; al[k] = WENO5_D[k] / (t * t); s += al[k]; }
+    for (int k = 0; k < 3; ++k) omega[k] = al[k] / s;
+}
 // interface flux of O6 for one 8-cell window: U[8][nf] row-major (cells i-3..i+4), direction d
+void oracle_interface_flux_order(int d, int nf, const double* Uwin, double alpha, double eps, double e_floor, double delta,
+                                 int order, double* Fhat) {
+    double Uw[8][5]; Prim<double> Pw[8];
+    for (int m = 0; m < 8; ++m) {
+        for (int q = 0; q < 5; ++q) Uw[m][q] = q < nf ? Uwin[m * nf + q] : 0.0;
+        Pw[m] = con2prim<double>(Uw[m][0], Uw[m][1], Uw[m][2], Uw[m][3], Uw[m][4], e_floor, delta);
+    }
+    double F[5];
+    interface_flux<double>(d, nf, Uw, Pw, alpha, eps, F, order);
+    for (int q = 0; q < nf; ++q) Fhat[q] = F[q];
+}
 void oracle_interface_flux(int d, int nf, const double* Uwin, double alpha, double eps, double e_floor, double delta,
                            double* Fhat) {
     double Uw[8][5]; Prim<double> Pw[8];

@@ -58,6 +58,12 @@ def lib():
         L.oracle_weno7.argtypes = [dp, d]
         L.oracle_weno7_parts.argtypes = [dp, d, dp, dp, dp, dp]
         L.oracle_interface_flux.argtypes = [i, i, dp, d, d, d, d, dp]
+        L.oracle_interface_flux_order.argtypes = [i, i, dp, d, d, d, d, i, dp]
+        L.oracle_set_weno_order.restype = i
+        L.oracle_set_weno_order.argtypes = [p, i]
+        L.oracle_weno5.restype = d
+        L.oracle_weno5.argtypes = [dp, d]
+        L.oracle_weno5_parts.argtypes = [dp, d, dp, dp, dp]
         L.oracle_source_q.restype = d
         L.oracle_source_q.argtypes = [d] * 5
         L.oracle_jet_axis_index.restype = i
@@ -79,12 +85,14 @@ class Oracle:
     """One CPU solver instance.  U arrays have shape (nf, nz, ny, nx), float64, x fastest."""
 
     def __init__(self, nx, ny, nz, dx, dt, nfields=4, weno_eps=WENO_EPS, v_cap_delta=V_CAP_DELTA,
-                 e_floor=E_FLOOR):
+                 e_floor=E_FLOOR, weno_order=7):
         self.L = lib()
         self.shape = (nfields, nz, ny, nx)
         self.h = self.L.oracle_create(nx, ny, nz, dx, dt, nfields, weno_eps, v_cap_delta, e_floor)
         if not self.h:
             raise ValueError("oracle_create: bad arguments")
+        if self.L.oracle_set_weno_order(self.h, weno_order):
+            raise ValueError("weno_order must be 5 or 7")
         self.njets = 0
 
     def close(self):
@@ -164,6 +172,20 @@ def weno7(v, eps=WENO_EPS):
     v = np.ascontiguousarray(v, dtype=np.float64)
     assert v.shape == (7,)
     return lib().oracle_weno7(_dp(v), eps)
+
+
+def weno5(v, eps=WENO_EPS):
+    """r = 3 reconstruction at the right face of the centre cell of the 5 values v."""
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    assert v.shape == (5,)
+    return lib().oracle_weno5(_dp(v), eps)
+
+
+def weno5_parts(v, eps=WENO_EPS):
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    q, beta, om = np.zeros(3), np.zeros(3), np.zeros(3)
+    lib().oracle_weno5_parts(_dp(v), eps, _dp(q), _dp(beta), _dp(om))
+    return q, beta, om
 
 
 def weno7_parts(v, eps=WENO_EPS):
