@@ -46,6 +46,7 @@ typedef struct {
     double weno_eps;     /* epsilon of the WENO-JS weights, default 1e-6 (R3) */
     double v_cap_delta;  /* |M| <= (1 - delta) E in con2prim, default 1e-10 (fp64) / 1e-5 (fp32) (R9, R10) */
     double e_floor;      /* E >= e_floor in con2prim, default 1e-12 GeV/fm^3 (R9) */
+    int    weno_order;   /* 7 (or 0): 7th-order WENO, the scheme the paper uses; 5: its 5th-order variant */
 } hydro_eos_t;
 
 /* Kernel classes timed by hydro_set_profiling / hydro_get_kernel_times. */
@@ -105,8 +106,8 @@ int hydro_get_last_stage_q(hydro_t *h, int jet, double out[3]);
 int hydro_set_profiling(hydro_t *h, int enable);
 int hydro_get_kernel_times(hydro_t *h, double ms[HYDRO_K_COUNT], long long launches[HYDRO_K_COUNT]);
 
-/* Which sweep kernels this handle uses: 1 = TMA ring kernels (fp64 and even nx: hydro_sweep_ring.cuh), 0 = generic
- * direct-load kernels (fp32, or odd nx where rows are not 16-byte aligned).  Same arithmetic either way. */
+/* Which sweep kernels this handle uses: always 1 = the TMA ring kernels of hydro_sweep_ring.cuh (rows are stored
+ * with a 16-byte-aligned pitch on the device, so every nx qualifies). */
 int hydro_sweep_path(const hydro_t *h);
 
 /* Number of kernel launches hydro_step has enqueued on this handle since create. */

@@ -17,8 +17,9 @@
 using namespace hydro_dev;
 
 struct hydro {
-    int nx, ny, nz, nf, prec;
-    long long N;
+    int nx, ny, nz, nf, prec, order;    // order: 7 (WENO7, the paper's scheme) or 5 (its WENO5 variant)
+    int nxp;                            // row pitch in reals: nx rounded up so that a row is a multiple of 16 bytes (TMA)
+    long long N, Np;                    // interior cells; field stride nxp*ny*nz
     double dx, dt, weno_eps, delta, e_floor;
     size_t esz;                         // bytes per real
     cudaStream_t stream;
@@ -36,9 +37,7 @@ struct hydro {
     long long step;
     int prim_slot;                      // DiagSlot holding alpha of buf[cur]'s primitives
     bool prims_valid;
-    int nseg[3];
     // ring sweeps (fp64, even nx): tensor maps per buffer and direction, march cells per block
-    bool use_tma;
     CUtensorMap mapU[3][3], mapW[3], mapP[3], mapL[3];
     int seg_len[3], tma_nseg[3];
     int num_sms;
@@ -102,7 +101,7 @@ template <typename R>
 int launch_prim(hydro* h, const void* U, int slot) {
     CK(cudaMemsetAsync(&h->diag->slot[slot], 0, sizeof(DiagSlot), h->stream));
     PrimArgs<R> a;
-    a.U = (const R*)U; a.P = (R*)h->P; a.W = (R*)h->W; a.diag = h->diag; a.slot = slot; a.N = h->N;
+    a.U = (const R*)U; a.P = (R*)h->P; a.W = (R*)h->W; a.diag = h->diag; a.slot = slot; a.N = h->N; a.Np = h->Np; a.nx = h->nx; a.nxp = h->nxp;
     a.e_floor = (R)h->e_floor; a.one_minus_delta = (R)(1.0 - h->delta);
     long long blocks = (h->N + 255) / 256;
     long long cap = (long long)h->num_sms * 8;
@@ -180,7 +179,7 @@ int make_map(hydro* h, CUtensorMap* out, void* base, int nfb, const unsigned box
     }
     cuuint64_t gdim[4] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny, (cuuint64_t)h->nz, (cuuint64_t)nfb};
     const cuuint64_t es8 = (cuuint64_t)h->esz;
-    cuuint64_t gstr[3] = {(cuuint64_t)h->nx * es8, (cuuint64_t)h->nx * h->ny * es8, (cuuint64_t)h->N * es8};
+    cuuint64_t gstr[3] = {(cuuint64_t)h->nxp * es8, (cuuint64_t)h->nxp * h->ny * es8, (cuuint64_t)h->Np * es8};
     cuuint32_t bx[4] = {box[0], box[1], box[2], box[3]};
     cuuint32_t es[4] = {1, 1, 1, 1};
     // x sweep boxes (8 cells of x innermost = 64 bytes in fp64, 32 bytes in fp32) are swizzled at their own width
@@ -234,21 +233,6 @@ int setup_tma(hydro* h) {
     return HYDRO_OK;
 }
 
-template <typename R, int DIR, int MODE>
-int launch_sweep(hydro* h, SweepArgs<R> a) {
-    const int nd = DIR == 0 ? h->nx : DIR == 1 ? h->ny : h->nz;
-    const long long ntrans = h->N / nd;
-    a.nseg = h->nseg[DIR];
-    dim3 grid((unsigned)((ntrans + 127) / 128), (unsigned)h->nf, (unsigned)a.nseg);
-    {
-        Timer t(h, HYDRO_K_SWEEP_X + DIR);
-        k_sweep<R, DIR, MODE><<<grid, 128, 0, h->stream>>>(a);
-    }
-    h->launches += 1;
-    CK(cudaGetLastError());
-    return HYDRO_OK;
-}
-
 template <typename R>
 int upload_jets(hydro* h) {
     if (!h->jets_dirty) return HYDRO_OK;
@@ -266,7 +250,7 @@ int launch_source(hydro* h, int slot, int stage, double stage_c, bool commit, do
     if ((rc = upload_jets<R>(h)) != HYDRO_OK) return rc;
     SourceArgs s;
     s.diag = h->diag; s.jets = h->jets_dev; s.njets = (int)h->jets.size(); s.slot = slot; s.stage = stage;
-    s.commit = commit ? 1 : 0; s.nx = h->nx; s.ny = h->ny; s.nz = h->nz; s.N = h->N; s.step = h->step;
+    s.commit = commit ? 1 : 0; s.nx = h->nx; s.ny = h->ny; s.nz = h->nz; s.nxp = h->nxp; s.N = h->Np; s.step = h->step;
     s.stage_c = stage_c; s.dx = h->dx; s.dt = h->dt; s.rk_weight = rk_weight; s.scale = scale;
     {
         Timer t(h, HYDRO_K_SOURCE);
@@ -301,26 +285,11 @@ int eval_stage_ring(hydro* h, const void* Uin, int slot, int stage, double stage
     return launch_ring<R, 2, OUT_REDUCE>(h, Uin, slot, &h->mapL[2], 0, hid, 0.0, 0.0);
 }
 
-// L(U_in, t_n + stage_c dt) into h->L; if Uout != 0 the stage combination forms the next stage state.
+// L(U_in, t_n + stage_c dt) into h->L; if Uout != 0 the stage combination forms the next stage state instead.
 template <typename R>
 int eval_stage(hydro* h, const void* Uin, int slot, int stage, double stage_c, bool commit, double rk_weight,
                void* Uout, const void* Un, double rk_a, double rk_b) {
-    if (h->use_tma) return eval_stage_ring<R>(h, Uin, slot, stage, stage_c, commit, rk_weight, Uout, Un, rk_a, rk_b);
-    SweepArgs<R> a;
-    a.U = (const R*)Uin; a.P = (const R*)h->P; a.W = (const R*)h->W; a.L = (R*)h->L;
-    a.Un = (const R*)Un; a.Uout = (R*)Uout; a.diag = h->diag; a.slot = slot;
-    a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.nf = h->nf; a.nseg = 1; a.use_un = Un != 0; a.seg_len = 0;
-    a.N = h->N;
-    a.eps_eff = (R)(144.0 * h->weno_eps);
-    a.half_inv_dx = (R)(0.5 / h->dx);
-    a.dt = (R)h->dt; a.rk_a = (R)rk_a; a.rk_b = (R)rk_b;
-    int rc;
-    if ((rc = launch_sweep<R, 0, 0>(h, a)) != HYDRO_OK) return rc;
-    if ((rc = launch_sweep<R, 1, 1>(h, a)) != HYDRO_OK) return rc;
-    if ((rc = launch_source<R>(h, slot, stage, stage_c, commit, rk_weight, h->L, 1.0)) != HYDRO_OK) return rc;
-    if (Uout) rc = launch_sweep<R, 2, 2>(h, a);
-    else rc = launch_sweep<R, 2, 1>(h, a);
-    return rc;
+    return eval_stage_ring<R>(h, Uin, slot, stage, stage_c, commit, rk_weight, Uout, Un, rk_a, rk_b);
 }
 
 template <typename R>
@@ -368,16 +337,18 @@ int prims_out_impl(hydro* h, void* out) {
     long long blocks = (h->N + 255) / 256;
     long long cap = (long long)h->num_sms * 8;
     if (blocks > cap) blocks = cap;
-    k_prims_out<R><<<(unsigned)blocks, 256, 0, h->stream>>>((const R*)h->buf[h->cur], (R*)out, h->N, h->nf,
+    k_prims_out<R><<<(unsigned)blocks, 256, 0, h->stream>>>((const R*)h->buf[h->cur], (R*)out, h->N, h->Np, h->nx, h->nxp, h->nf,
                                                             (R)h->e_floor, (R)(1.0 - h->delta));
     CK(cudaGetLastError());
     return HYDRO_OK;
 }
 
+// pitched device buffer (row pitch nxp) -> the caller's dense layout (row length nx), nf*nz*ny rows
 int copy_out(hydro* h, const void* dev_src, void* out, int memspace) {
-    const size_t bytes = (size_t)h->N * h->nf * h->esz;
-    CK(cudaMemcpyAsync(out, dev_src, bytes, memspace == HYDRO_MEM_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice,
-                       h->stream));
+    const cudaMemcpyKind kind = memspace == HYDRO_MEM_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+    const size_t row = (size_t)h->nx * h->esz, rows = (size_t)h->nf * h->nz * h->ny;
+    if (h->nxp == h->nx) CK(cudaMemcpyAsync(out, dev_src, row * rows, kind, h->stream));
+    else CK(cudaMemcpy2DAsync(out, row, dev_src, (size_t)h->nxp * h->esz, row, rows, kind, h->stream));
     CK(cudaStreamSynchronize(h->stream));
     return HYDRO_OK;
 }
@@ -391,27 +362,34 @@ int hydro_create(hydro_t** out, int nx, int ny, int nz, double dx, double dt, co
     *out = 0;
     hydro_eos_t o;
     o.eos = HYDRO_EOS_CONFORMAL; o.nfields = 4; o.precision = 64; o.weno_eps = 0; o.v_cap_delta = 0; o.e_floor = 0;
+    o.weno_order = 0;
     if (eos) o = *eos;
     if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0) || !(dt > 0) || !std::isfinite(dx) || !std::isfinite(dt)) return HYDRO_EINVAL;
     if (o.eos != HYDRO_EOS_CONFORMAL || (o.nfields != 4 && o.nfields != 5) || (o.precision != 64 && o.precision != 32))
         return HYDRO_EINVAL;
     if (o.weno_eps < 0 || o.v_cap_delta < 0 || o.v_cap_delta >= 1 || o.e_floor < 0) return HYDRO_EINVAL;
+    if (o.weno_order != 0 && o.weno_order != 5 && o.weno_order != 7) return HYDRO_EINVAL;
     if ((long long)nx * ny * nz > (1LL << 40)) return HYDRO_EINVAL;
     hydro* h = new (std::nothrow) hydro();
     if (!h) return HYDRO_ENOMEM;
     h->nx = nx; h->ny = ny; h->nz = nz; h->nf = o.nfields; h->prec = o.precision;
     h->N = (long long)nx * ny * nz;
+    h->order = o.weno_order == 5 ? 5 : 7;
     h->dx = dx; h->dt = dt;
     h->weno_eps = o.weno_eps > 0 ? o.weno_eps : 1e-6;
     h->delta = o.v_cap_delta > 0 ? o.v_cap_delta : (o.precision == 64 ? 1e-10 : 1e-5);
     h->e_floor = o.e_floor > 0 ? o.e_floor : 1e-12;
     h->esz = o.precision == 64 ? 8 : 4;
+    {
+        const int per16 = 16 / (int)h->esz;                             // reals per 16 bytes
+        h->nxp = (nx + per16 - 1) / per16 * per16;
+        h->Np = (long long)h->nxp * ny * nz;
+    }
     h->stream = (cudaStream_t)cuda_stream; h->own_stream = false;
     for (int b = 0; b < 3; ++b) h->buf[b] = 0;
     h->cur = 0; h->L = h->P = h->W = h->scratch = 0; h->diag = 0; h->jets_dev = 0;
     h->jets_dirty = false; h->step = 0; h->prim_slot = 0; h->prims_valid = false; h->launches = 0;
     h->profiling = false;
-    h->use_tma = false;
     for (int k = 0; k < HYDRO_K_COUNT; ++k) { h->k_ms[k] = 0; h->k_n[k] = 0; }
     int rc = HYDRO_OK;
     do {
@@ -425,31 +403,21 @@ int hydro_create(hydro_t** out, int nx, int ny, int nz, double dx, double dt, co
             if (e != cudaSuccess) { rc = cuda_fail(h, e, "cudaStreamCreate"); break; }
             h->own_stream = true;
         }
-        const size_t fb = (size_t)h->N * h->nf * h->esz;
+        const size_t fb = (size_t)h->Np * h->nf * h->esz;
         void** ptrs[] = {&h->buf[0], &h->buf[1], &h->buf[2], &h->L};
         for (int b = 0; b < 4 && rc == HYDRO_OK; ++b) {
             e = cudaMalloc(ptrs[b], fb);
             if (e != cudaSuccess) rc = cuda_fail(h, e, "cudaMalloc(state)");
+            else if (h->nxp != h->nx && (e = cudaMemsetAsync(*ptrs[b], 0, fb, h->stream)) != cudaSuccess)
+                rc = cuda_fail(h, e, "cudaMemset(state)");           // pad columns: finite, never cells
         }
         if (rc != HYDRO_OK) break;
-        if ((e = cudaMalloc(&h->P, (size_t)h->N * h->esz)) != cudaSuccess) { rc = cuda_fail(h, e, "cudaMalloc(P)"); break; }
-        if ((e = cudaMalloc(&h->W, (size_t)h->N * h->esz)) != cudaSuccess) { rc = cuda_fail(h, e, "cudaMalloc(W)"); break; }
+        if ((e = cudaMalloc(&h->P, (size_t)h->Np * h->esz)) != cudaSuccess) { rc = cuda_fail(h, e, "cudaMalloc(P)"); break; }
+        if ((e = cudaMalloc(&h->W, (size_t)h->Np * h->esz)) != cudaSuccess) { rc = cuda_fail(h, e, "cudaMalloc(W)"); break; }
         if ((e = cudaMalloc((void**)&h->diag, sizeof(Diag))) != cudaSuccess) { rc = cuda_fail(h, e, "cudaMalloc(diag)"); break; }
         if ((e = cudaMalloc((void**)&h->jets_dev, sizeof(JetDev) * MAX_JETS)) != cudaSuccess) { rc = cuda_fail(h, e, "cudaMalloc(jets)"); break; }
         if ((e = cudaMemsetAsync(h->diag, 0, sizeof(Diag), h->stream)) != cudaSuccess) { rc = cuda_fail(h, e, "cudaMemset(diag)"); break; }
-        // segments along the march axis: enough threads to fill the machine on small grids
-        const int nd[3] = {nx, ny, nz};
-        for (int d = 0; d < 3; ++d) {
-            long long threads = (h->N / nd[d]) * h->nf;
-            int seg = 1;
-            while (threads * seg < (long long)h->num_sms * 1024 && nd[d] / (seg * 2) >= 16) seg *= 2;
-            h->nseg[d] = seg;
-        }
-        // TMA-staged sweeps need 16-byte global strides (nx even in fp64, a multiple of 4 in fp32);
-        // HYDRO_NO_TMA=1 forces the direct-load kernels
-        const char* no_tma = getenv("HYDRO_NO_TMA");
-        h->use_tma = (nx * (int)h->esz) % 16 == 0 && !(no_tma && no_tma[0] == '1');
-        if (h->use_tma) rc = setup_tma(h);
+        rc = setup_tma(h);
     } while (0);
     if (rc != HYDRO_OK) {
         // keep the error text out of reach of the caller: handle is destroyed
@@ -473,9 +441,10 @@ void hydro_destroy(hydro_t* h) {
 
 int hydro_set_state(hydro_t* h, const void* U, int memspace) {
     if (!h || !U || (memspace != HYDRO_MEM_HOST && memspace != HYDRO_MEM_DEVICE)) return HYDRO_EINVAL;
-    const size_t bytes = (size_t)h->N * h->nf * h->esz;
-    CK(cudaMemcpyAsync(h->buf[h->cur], U, bytes, memspace == HYDRO_MEM_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice,
-                       h->stream));
+    const cudaMemcpyKind kind = memspace == HYDRO_MEM_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+    const size_t row = (size_t)h->nx * h->esz, rows = (size_t)h->nf * h->nz * h->ny;
+    if (h->nxp == h->nx) CK(cudaMemcpyAsync(h->buf[h->cur], U, row * rows, kind, h->stream));
+    else CK(cudaMemcpy2DAsync(h->buf[h->cur], (size_t)h->nxp * h->esz, U, row, row, rows, kind, h->stream));
     CK(cudaMemsetAsync(h->diag, 0, sizeof(Diag), h->stream));
     if (memspace == HYDRO_MEM_HOST) CK(cudaStreamSynchronize(h->stream));
     h->step = 0;
@@ -523,13 +492,13 @@ int hydro_get_fields(hydro_t* h, void* out, int which, int memspace) {
     if (!h || !out || (memspace != HYDRO_MEM_HOST && memspace != HYDRO_MEM_DEVICE)) return HYDRO_EINVAL;
     if (which == HYDRO_FIELDS_CONSERVED) return copy_out(h, h->buf[h->cur], out, memspace);
     if (which != HYDRO_FIELDS_PRIMITIVE) return HYDRO_EINVAL;
-    if (memspace == HYDRO_MEM_DEVICE) {
+    if (memspace == HYDRO_MEM_DEVICE && h->nxp == h->nx) {
         int rc = h->prec == 64 ? prims_out_impl<double>(h, out) : prims_out_impl<float>(h, out);
         if (rc != HYDRO_OK) return rc;
         CK(cudaStreamSynchronize(h->stream));
         return HYDRO_OK;
     }
-    // host destination: stage through the RHS buffer (free between steps)
+    // host destination or pitched rows: stage through the RHS buffer (free between steps)
     int rc = h->prec == 64 ? prims_out_impl<double>(h, h->L) : prims_out_impl<float>(h, h->L);
     if (rc != HYDRO_OK) return rc;
     return copy_out(h, h->L, out, memspace);
@@ -592,7 +561,7 @@ int hydro_get_kernel_times(hydro_t* h, double ms[HYDRO_K_COUNT], long long launc
 
 long long hydro_launch_count(const hydro_t* h) { return h ? h->launches : -1; }
 
-int hydro_sweep_path(const hydro_t* h) { return h && h->use_tma ? 1 : 0; }
+int hydro_sweep_path(const hydro_t* h) { return h ? 1 : 0; }
 
 int hydro_measure_alu_peak(int precision, double millis, void* cuda_stream, double* tflops) {
     if (!tflops || (precision != 64 && precision != 32) || !(millis > 0)) return HYDRO_EINVAL;

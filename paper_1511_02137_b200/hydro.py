@@ -30,7 +30,7 @@ SYMBOLS = ("hydro_create", "hydro_destroy", "hydro_set_state", "hydro_add_jet", 
 
 class EosT(C.Structure):
     _fields_ = [("eos", C.c_int), ("nfields", C.c_int), ("precision", C.c_int), ("weno_eps", C.c_double),
-                ("v_cap_delta", C.c_double), ("e_floor", C.c_double)]
+                ("v_cap_delta", C.c_double), ("e_floor", C.c_double), ("weno_order", C.c_int)]
 
 
 class HydroError(RuntimeError):
@@ -123,13 +123,13 @@ class Hydro:
     """One solver handle (hydro_t).  Arrays have shape (nfields, nz, ny, nx), x fastest."""
 
     def __init__(self, nx, ny, nz, dx, dt, nfields=4, precision=64, weno_eps=0.0, v_cap_delta=0.0, e_floor=0.0,
-                 stream=None):
+                 stream=None, weno_order=7):
         self.L = load()
         self.h = C.c_void_p()
         self.shape = (nfields, nz, ny, nx)
         self.nfields = nfields
         self.dtype = np.float64 if precision == 64 else np.float32
-        eos = EosT(0, nfields, precision, weno_eps, v_cap_delta, e_floor)
+        eos = EosT(0, nfields, precision, weno_eps, v_cap_delta, e_floor, weno_order)
         self._stream = stream                      # keep a torch stream object alive
         sp = 0
         if stream is not None:

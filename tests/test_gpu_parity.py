@@ -290,7 +290,7 @@ def test_fp32_rhs_single_stage(H, oracle, n, nf):
     U0 = S.make_state(c).astype(np.float32)
     g = H.Hydro(*n, c["dx"], c["dt"], nfields=nf, precision=32)
     o = oracle.Oracle(*n, c["dx"], c["dt"], nfields=nf, v_cap_delta=1e-5)
-    assert g.uses_ring() == (n[0] % 4 == 0)
+    assert g.uses_ring()
     g.set_state(U0)
     o.set_state(U0.astype(np.float64))
     for pos, d in c["jets"]:
