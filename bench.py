@@ -41,6 +41,9 @@ UNIT = "cell-updates/s"
 # Of these the sweep kernels carry interface_flux + divergence (+ the stage combination in the last sweep).
 FLOPS_STAGE = {4: 3764.0, 5: 4691.0}
 FLOPS_SWEEPS_STAGE = {4: 3 * (1208.0 + 12.0) + 20.0, 5: 3 * (1510.0 + 15.0) + 25.0}
+# the WENO5 variant (--weno-order 5), same counting (oracle_count_flops_order)
+FLOPS_STAGE_W5 = {4: 1820.0, 5: 2261.0}
+FLOPS_SWEEPS_STAGE_W5 = {4: 3 * (560.0 + 12.0) + 20.0, 5: 3 * (700.0 + 15.0) + 25.0}
 FP64_NOMINAL_TF = 148 * 64 * 2 * 1.965e9 / 1e12          # 148 SMs x 64 DFMA/clk x 2 x 1.965 GHz = 37.2
 # dram__bytes_read.sum + dram__bytes_write.sum per sweep launch at 256^3 fp64 nf=4, mean of the x (COMBINE), y and z
 # (REDUCE) kernels, from the one `ncu --set full` capture summarised in profiles/r1_c_ring_ncu_summary.txt
@@ -113,14 +116,14 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_slab_run(cfg, nzs, steps, warmup=0):
+def oracle_slab_run(cfg, nzs, steps, warmup=0, order=7):
     """Oracle on the central nzs planes of config `cfg`'s initial condition; returns (cells, seconds, threads)."""
     from oracle import oracle as O
     c = S.CONFIGS[cfg]
     nx, ny, nz = c["n"]
     k0 = nz // 2 - nzs // 2
     U0 = S.make_state(cfg, z_range=(k0, k0 + nzs))
-    o = O.Oracle(nx, ny, nzs, c["dx"], c["dt"], nfields=c["nf"])
+    o = O.Oracle(nx, ny, nzs, c["dx"], c["dt"], nfields=c["nf"], weno_order=order)
     o.set_state(U0)
     for pos, d in c["jets"]:
         o.add_jet(pos, d, S.KAPPA_RAD, S.KAPPA_COLL, S.CR_OVER_CF)
@@ -140,10 +143,10 @@ def run_reference(args, rank):
     cfg = args.config
     c = S.CONFIGS[cfg]
     # size the slab so that (K + W) steps take about two minutes: calibrate on one step of 8 planes
-    cells8, t8, threads = oracle_slab_run(cfg, 8, 1)
+    cells8, t8, threads = oracle_slab_run(cfg, 8, 1, order=args.weno_order)
     budget = 120.0
     nzs = int(min(c["n"][2], max(8, 8 * int(budget / (t8 * (args.steps + args.warmup)) + 1e-9))))
-    cells, secs, threads = oracle_slab_run(cfg, nzs, args.steps, args.warmup)
+    cells, secs, threads = oracle_slab_run(cfg, nzs, args.steps, args.warmup, order=args.weno_order)
     value = cells * args.steps / secs
     sample = "%dx%dx%d central slab of config %d's IC + jet, %d RK3 steps" % (c["n"][0], c["n"][1], nzs, cfg,
                                                                               args.steps)
@@ -163,7 +166,7 @@ def workload_config(args, cfg):
     return {"workload": "BASELINE config %d: %dx%dx%d, dx=%g fm, dt=%g fm/c, nf=%d, p=e/3, ellipsoidal flow + %d jet(s), "
                         "outflow ghosts" % (cfg, c["n"][0], c["n"][1], c["n"][2], c["dx"], c["dt"], c["nf"],
                                             len(c["jets"])),
-            "cells": int(np.prod(c["n"])), "config_steps": c["steps"],
+            "cells": int(np.prod(c["n"])), "config_steps": c["steps"], "weno_order": getattr(args, "weno_order", 7),
             "parallelism": "replicas x%d" % args.gpus,
             "l2": "state (%.0f MiB per copy) exceeds L2; no flush needed" %
                   (np.prod(c["n"]) * c["nf"] * (args.precision // 8) / 2 ** 20)}
@@ -177,6 +180,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
+    ap.add_argument("--weno-order", type=int, default=7, choices=[7, 5])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -215,7 +219,8 @@ def main():
     with torch.cuda.stream(stream):
         U0d = U0h.cuda(non_blocking=True)
     stream.synchronize()
-    g = H.Hydro(*c["n"], c["dx"], c["dt"], nfields=c["nf"], precision=args.precision, stream=stream)
+    g = H.Hydro(*c["n"], c["dx"], c["dt"], nfields=c["nf"], precision=args.precision, stream=stream,
+                weno_order=args.weno_order)
     for pos, d in c["jets"]:
         g.add_jet(pos, d, S.KAPPA_RAD, S.KAPPA_COLL, S.CR_OVER_CF)
 
@@ -274,11 +279,12 @@ def main():
         sw_n = sum(k["launches"] for k in sweeps)
         all_ms = sum(k["ms"] for k in kt.values())
         # dominant kernel class: the WENO7-LF sweep kernels; flops per launch = (sweep flops per cell per stage / 3) * cells
-        fl_launch = FLOPS_SWEEPS_STAGE[nf] / 3.0 * cells
+        fl_sweeps = (FLOPS_SWEEPS_STAGE if args.weno_order == 7 else FLOPS_SWEEPS_STAGE_W5)[nf]
+        fl_stage = (FLOPS_STAGE if args.weno_order == 7 else FLOPS_STAGE_W5)[nf]
+        fl_launch = fl_sweeps / 3.0 * cells
         achieved = fl_launch / (sw_ms / sw_n * 1e-3) / 1e12 if sw_n else 0.0
         nominal = FP64_NOMINAL_TF * (1 if args.precision == 64 else 2)
-        roof = {"bound": "alu", "kernel": "k_sweep_ring<x|y|z> (WENO7-LF flux + divergence + RK3 combine)" if g.uses_ring() else
-                          "k_sweep<x|y|z> (generic path)",
+        roof = {"bound": "alu", "kernel": "k_sweep_ring<x|y|z> (WENO%d-LF flux + divergence + RK3 combine)" % args.weno_order,
                 "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf,
                 "peak_kind": "measured in this run: register-resident %s chain on all SMs (hydro_measure_alu_peak)" %
                              ("DFMA" if args.precision == 64 else "FFMA"),
@@ -286,8 +292,8 @@ def main():
                 "flops_per_launch": fl_launch, "avg_launch_ms": sw_ms / sw_n if sw_n else None,
                 "share_of_step": sw_ms / all_ms if all_ms else None,
                 "kernel_ms_per_step": {k: v["ms"] / args.steps for k, v in kt.items()},
-                "whole_path_frac": (FLOPS_STAGE[nf] * 3 * value) / (peak_tf * 1e12),
-                "traffic": NCU_TRAFFIC_SWEEP_256_F64_NF4 if (cfg == 3 and args.precision == 64 and g.uses_ring()) else None,
+                "whole_path_frac": (fl_stage * 3 * value) / (peak_tf * 1e12),
+                "traffic": NCU_TRAFFIC_SWEEP_256_F64_NF4 if (cfg == 3 and args.precision == 64 and args.weno_order == 7) else None,
                 "traffic_source": "profiles/r1_c_ring_ncu_summary.txt (ncu --set full, dram read+write per launch)",
                 "algorithmic_bytes_per_launch": (nf + 2 + nf + nf * 2.0 / 9.0 + 2.0 / 3.0 * nf) * 8.0 * cells}
         line = {
@@ -304,7 +310,7 @@ def main():
                            "what": "hydro_set_state(host) + hydro_step(K) + hydro_get_fields(host), pinned buffers; "
                                    "bytes are the one upload / one download spread over K steps"}
         if not args.no_cpu_baseline and world == 1:
-            cells_s, secs, threads = oracle_slab_run(cfg, 16, 2)
+            cells_s, secs, threads = oracle_slab_run(cfg, 16, 2, order=args.weno_order)
             line["cpu_baseline"] = {"value": cells_s * 2 / secs, "unit": UNIT, "cores": threads, "kind": "oracle",
                                     "sample": "%dx%dx16 central slab of config %d's IC + jet, 2 RK3 steps (%.1f s)" %
                                               (c["n"][0], c["n"][1], cfg, secs)}

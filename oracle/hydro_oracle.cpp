@@ -544,7 +544,7 @@ void oracle_constants(double out[3]) { out[0] = HBARC; out[1] = G_DOF; out[2] = 
 // once per cell] + the divergence update) + RK combine.  Returns flops per cell per stage.
 // breakdown[0]=con2prim, [1]=wavespeeds, [2]=one interface flux (nf fields, incl. split),
 // [3]=divergence per direction, [4]=RK combine (worst stage), [5]=one weno7 reconstruction.
-double oracle_count_flops(int nf, double* breakdown) {
+double oracle_count_flops_order(int nf, int order, double* breakdown) {
     typedef Counted R;
     R Uw[8][5]; Prim<R> Pw[8];
     for (int m = 0; m < 8; ++m) {
@@ -565,10 +565,11 @@ double oracle_count_flops(int nf, double* breakdown) {
     // which is the oracle's redundancy, not the algorithm's: count 1/8 of the split work.
     t0 = Counted::ops;
     R Fh[5];
-    interface_flux<R>(0, nf, Uw, Pw, R(0.9), 1e-6, Fh);
+    interface_flux<R>(0, nf, Uw, Pw, R(0.9), 1e-6, Fh, order);
     long long c_if_all = Counted::ops - t0;
     t0 = Counted::ops;
-    R w = weno7<R>(Uw[0][0], Uw[1][0], Uw[2][0], Uw[3][0], Uw[4][0], Uw[5][0], Uw[6][0], 1e-6);
+    R w = order == 5 ? weno5<R>(Uw[0][0], Uw[1][0], Uw[2][0], Uw[3][0], Uw[4][0], 1e-6)
+                     : weno7<R>(Uw[0][0], Uw[1][0], Uw[2][0], Uw[3][0], Uw[4][0], Uw[5][0], Uw[6][0], 1e-6);
     long long c_weno = Counted::ops - t0;
     (void)w;
     long long c_split_all = c_if_all - 2LL * nf * c_weno - nf;    // 8 cells' flux+split
@@ -583,6 +584,8 @@ double oracle_count_flops(int nf, double* breakdown) {
     }
     return total;
 }
+
+double oracle_count_flops(int nf, double* breakdown) { return oracle_count_flops_order(nf, 7, breakdown); }
 
 int oracle_num_threads(void) {
 #ifdef _OPENMP

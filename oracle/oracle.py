@@ -71,6 +71,8 @@ def lib():
         L.oracle_constants.argtypes = [dp]
         L.oracle_count_flops.restype = d
         L.oracle_count_flops.argtypes = [i, dp]
+        L.oracle_count_flops_order.restype = d
+        L.oracle_count_flops_order.argtypes = [i, i, dp]
         L.oracle_num_threads.restype = i
         L.oracle_set_num_threads.argtypes = [i]
         _lib = L
@@ -218,9 +220,9 @@ def constants():
     return dict(hbarc=out[0], g=out[1], cs2=out[2])
 
 
-def count_flops(nf=4):
+def count_flops(nf=4, order=7):
     br = np.zeros(6)
-    tot = lib().oracle_count_flops(nf, _dp(br))
+    tot = lib().oracle_count_flops_order(nf, order, _dp(br))
     return tot, dict(con2prim=br[0], wavespeeds=br[1], interface_flux=br[2], divergence=br[3], rk=br[4],
                      weno7=br[5])
 

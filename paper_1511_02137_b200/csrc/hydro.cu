@@ -122,7 +122,7 @@ int buf_index(const hydro* h, const void* U) {
 
 // One ring sweep (hydro_sweep_ring.cuh).  `Us` must be one of the three state buffers; `out_map` is the tensor map
 // (for direction DIR) of the buffer the result is stored / reduced into; `un_map` that of U^n (OUT_COMBINE).
-template <typename R, int DIR, int OUT, int NF>
+template <typename R, int ORDER, int DIR, int OUT, int NF>
 int launch_ring_nf(hydro* h, const void* Us, int slot, const CUtensorMap* out_map, const CUtensorMap* un_map, double coef,
                    double rk_a, double rk_b) {
     const int b = buf_index(h, Us);
@@ -131,14 +131,14 @@ int launch_ring_nf(hydro* h, const void* Us, int slot, const CUtensorMap* out_ma
     m.U = h->mapU[b][DIR]; m.W = h->mapW[DIR]; m.P = h->mapP[DIR]; m.Out = *out_map; m.Un = un_map ? *un_map : *out_map;
     RingArgs a;
     a.diag = h->diag; a.slot = slot; a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.seg_len = h->seg_len[DIR];
-    a.eps_eff = 144.0 * h->weno_eps; a.coef = coef; a.dt = h->dt; a.rk_a = rk_a; a.rk_b = rk_b;
+    a.eps_eff = (ORDER == 5 ? 48.0 : 144.0) * h->weno_eps; a.coef = coef; a.dt = h->dt; a.rk_a = rk_a; a.rk_b = rk_b;
     const int nlane = DIR == 0 ? h->ny : h->nx;
     const int other = DIR == 2 ? h->ny : h->nz;
     dim3 grid((unsigned)(((nlane + 31) / 32) * other), (unsigned)h->tma_nseg[DIR], 1);
     dim3 block(32, NF, 1);
     {
         Timer t(h, HYDRO_K_SWEEP_X + DIR);
-        k_sweep_ring<R, DIR, OUT, NF><<<grid, block, ring_smem_bytes(NF, OUT, sizeof(R)), h->stream>>>(m, a);
+        k_sweep_ring<R, ORDER, DIR, OUT, NF><<<grid, block, ring_smem_bytes(NF, OUT, sizeof(R)), h->stream>>>(m, a);
     }
     h->launches += 1;
     CK(cudaGetLastError());
@@ -148,14 +148,19 @@ int launch_ring_nf(hydro* h, const void* Us, int slot, const CUtensorMap* out_ma
 template <typename R, int DIR, int OUT>
 int launch_ring(hydro* h, const void* Us, int slot, const CUtensorMap* out_map, const CUtensorMap* un_map, double coef,
                 double rk_a, double rk_b) {
-    return h->nf == 4 ? launch_ring_nf<R, DIR, OUT, 4>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b)
-                      : launch_ring_nf<R, DIR, OUT, 5>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b);
+    if (h->order == 5)
+        return h->nf == 4 ? launch_ring_nf<R, 5, DIR, OUT, 4>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b)
+                          : launch_ring_nf<R, 5, DIR, OUT, 5>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b);
+    return h->nf == 4 ? launch_ring_nf<R, 7, DIR, OUT, 4>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b)
+                      : launch_ring_nf<R, 7, DIR, OUT, 5>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b);
 }
 
 template <typename R, int DIR, int OUT, int NF>
 int set_smem_attr() {
-    return cudaFuncSetAttribute(k_sweep_ring<R, DIR, OUT, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                ring_smem_bytes(NF, OUT, sizeof(R))) == cudaSuccess ? 0 : 1;
+    return (cudaFuncSetAttribute(k_sweep_ring<R, 7, DIR, OUT, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 ring_smem_bytes(NF, OUT, sizeof(R))) == cudaSuccess ? 0 : 1) +
+           (cudaFuncSetAttribute(k_sweep_ring<R, 5, DIR, OUT, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 ring_smem_bytes(NF, OUT, sizeof(R))) == cudaSuccess ? 0 : 1);
 }
 template <typename R, int NF>
 int set_smem_attrs() {

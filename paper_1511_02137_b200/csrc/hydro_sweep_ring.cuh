@@ -111,7 +111,7 @@ struct RingArgs {
     int slot;                  // which DiagSlot holds alpha of U_s
     int nx, ny, nz;
     int seg_len;               // march cells per block (multiple of RING_CH)
-    double eps_eff;            // 144 * weno_eps: the split fluxes are carried as 2 f^+-, beta as 36 beta
+    double eps_eff;            // WENO7: 144 * weno_eps (the split fluxes are carried as 2 f^+-, beta as 36 beta); WENO5: 48 * weno_eps
     double coef;               // OUT_STORE / OUT_REDUCE: c = [b dt] / (2 dx);  OUT_COMBINE*: 1 / (2 dx)
     double dt, rk_a, rk_b;
 };
@@ -143,18 +143,20 @@ struct RotWin {
     }
 };
 
-template <int r, typename R>
+template <int r, int ORDER, typename R>
 __device__ __forceinline__ void rot_push(RotWin<R>& w, R x, R c3, R eps) {
     constexpr int p = (r + 7) & 7;
     const R dn = x - w.V[p];
     const R en = dn - w.D[p];
-    const R tn = en - w.E[p];
-    w.G[r] = tn - w.T;
-    w.S[r] = Real<R>::fma_(c3 * tn, tn, eps);
+    if (ORDER == 7) {
+        const R tn = en - w.E[p];
+        w.G[r] = tn - w.T;
+        w.S[r] = Real<R>::fma_(c3 * tn, tn, eps);
+        w.T = tn;
+    }
     w.V[r] = x;
     w.D[r] = dn;
     w.E[r] = en;
-    w.T = tn;
 }
 
 // reciprocal of a normal, well-scaled double: hardware seed (the upper 32 bits of the operand and of the result,
@@ -213,13 +215,50 @@ __device__ __forceinline__ void weno7_diff(R D0, R D1, R D2, R E0, R E1, R E2, R
     base12 = lam0 + m0;                                   // 3 D_0 - 10 D_1 + 13 D_2 = lam_0 + m_0 identically
 }
 
+// One WENO5-JS reconstruction (r = 3) from the differences of the stencil values
+// x_0..x_4 (centre x_2), D_j = x_{j+1} - x_j, E_j = D_{j+1} - D_j:
+//   candidates   6 (q_0 - x_2) = 5 D_1 - 2 D_0,   6 (q_1 - q_0) = 2 (E_1 - E_0),   6 (q_2 - q_1) = -(E_2 - E_1)
+//   smoothness   12 beta_k + eps = 13 E_k^2 + 3 l_k^2 + eps,  l_0 = 3 D_1 - D_0,  l_1 = D_1 + D_2,  l_2 = 3 D_2 - D_3
+//   weights      omega_k ~ d_k / (eps + beta_k)^2,  d = (1, 6, 3)/10  (fp64: common denominator; fp32: reciprocals)
+// Returns base6 = 6 (q_0 - x_2) and num6/den = 6 sum_k omega_k (q_k - q_0):  W = x_2 + (base6 + num6/den)/6.
+template <typename R>
+__device__ __forceinline__ void weno5_diff(R D0, R D1, R D2, R D3, R E0, R E1, R E2, R eps, R& base6, R& num6, R& den) {
+    typedef Real<R> T;
+    const R l0 = T::fma_(R(3), D1, -D0);
+    const R l1 = D1 + D2;
+    const R l2 = T::fma_(R(3), D2, -D3);
+    const R b0 = T::fma_(R(13) * E0, E0, T::fma_(R(3) * l0, l0, eps));
+    const R b1 = T::fma_(R(13) * E1, E1, T::fma_(R(3) * l1, l1, eps));
+    const R b2 = T::fma_(R(13) * E2, E2, T::fma_(R(3) * l2, l2, eps));
+    R u0, u1, u2;
+    if (sizeof(R) == 8) {
+        const R t0 = b0 * b0, t1 = b1 * b1, t2 = b2 * b2;
+        u0 = t1 * t2; u1 = t0 * t2; u2 = t0 * t1;
+    } else {
+        const float r0 = rcp_ulp((float)b0), r1 = rcp_ulp((float)b1), r2 = rcp_ulp((float)b2);
+        u0 = r0 * r0; u1 = r1 * r1; u2 = r2 * r2;
+    }
+    const R a2 = R(3) * u2;
+    const R a12 = T::fma_(R(6), u1, a2);
+    den = u0 + a12;
+    num6 = T::fma_(a12, R(2) * (E1 - E0), -a2 * (E2 - E1));
+    base6 = T::fma_(R(5), D1, R(-2) * D0);
+}
+
 // 2 F_hat at the interface whose newest needed cell sits in slot r of both windows (plus side lags one slot):
 //   plus  side: cells i-3..i+3 = slots r-7..r-1, centre i   = V[r-4]
 //   minus side: cells i-2..i+4 = slots r-6..r,   centre i+1 = V[r-3], stencil order reversed (D_j = -d[5-j], ...)
-template <int r, typename R>
-__device__ __forceinline__ R rot_flux(const RotWin<R>& wp, const RotWin<R>& wm) {
+//   ORDER 5: plus cells i-2..i+2 = slots r-6..r-2 (centre V[r-4]); minus cells i-1..i+3 = slots r-5..r-1 reversed
+template <int r, int ORDER, typename R>
+__device__ __forceinline__ R rot_flux(const RotWin<R>& wp, const RotWin<R>& wm, R eps) {
 #define SL(k) (((r) + (k) + 16) & 7)
     R bp, np_, dp, bm, nm, dm;
+    if (ORDER == 5) {
+        weno5_diff<R>(wp.D[SL(-5)], wp.D[SL(-4)], wp.D[SL(-3)], wp.D[SL(-2)], wp.E[SL(-4)], wp.E[SL(-3)], wp.E[SL(-2)], eps,
+                      bp, np_, dp);
+        weno5_diff<R>(-wm.D[SL(-1)], -wm.D[SL(-2)], -wm.D[SL(-3)], -wm.D[SL(-4)], wm.E[SL(-1)], wm.E[SL(-2)], wm.E[SL(-3)],
+                      eps, bm, nm, dm);
+    } else {
     weno7_diff<R>(wp.D[SL(-6)], wp.D[SL(-5)], wp.D[SL(-4)],
                   wp.E[SL(-5)], wp.E[SL(-4)], wp.E[SL(-3)], wp.E[SL(-2)], wp.E[SL(-1)],
                   wp.S[SL(-4)], wp.S[SL(-3)], wp.S[SL(-2)], wp.S[SL(-1)],
@@ -228,10 +267,11 @@ __device__ __forceinline__ R rot_flux(const RotWin<R>& wp, const RotWin<R>& wm) 
                   wm.E[SL(0)], wm.E[SL(-1)], wm.E[SL(-2)], wm.E[SL(-3)], wm.E[SL(-4)],
                   wm.S[SL(0)], wm.S[SL(-1)], wm.S[SL(-2)], wm.S[SL(-3)],
                   wm.G[SL(0)], wm.G[SL(-1)], wm.G[SL(-2)], bm, nm, dm);
+    }
     R x;
     if (sizeof(R) == 8) x = (R)(fma((double)np_, (double)dm, (double)nm * (double)dp) * rcp_cubic((double)dp * (double)dm));
     else x = (R)fmaf((float)np_, rcp_ulp((float)dp), (float)nm * rcp_ulp((float)dm));
-    return Real<R>::fma_((bp + bm) + x, R(1.0 / 12.0), wp.V[SL(-4)] + wm.V[SL(-3)]);
+    return Real<R>::fma_((bp + bm) + x, ORDER == 5 ? R(1.0 / 6.0) : R(1.0 / 12.0), wp.V[SL(-4)] + wm.V[SL(-3)]);
 #undef SL
 }
 
@@ -254,7 +294,7 @@ struct RowPtr {
     }
 };
 
-template <typename R, int DIR, int OUT, int NF>
+template <typename R, int ORDER, int DIR, int OUT, int NF>
 struct SweepCtx {
     RotWin<R> wp, wm;
     R fhat_prev;
@@ -277,13 +317,13 @@ struct SweepCtx {
         const R md = pmd.template at<r>();
         const R B = T::fma_(md, pw.template at<r>(), kE);
         const R F = T::fma_(pa.template at<r>(), B, pp.template at<r>());
-        rot_push<r, R>(wp, T::fma_(alpha, u, F), c3, eps);
-        rot_push<r, R>(wm, T::fma_(-alpha, u, F), c3, eps);
+        rot_push<r, ORDER, R>(wp, T::fma_(alpha, u, F), c3, eps);
+        rot_push<r, ORDER, R>(wm, T::fma_(-alpha, u, F), c3, eps);
     }
     template <int r>
     __device__ __forceinline__ void emit() {
         typedef Real<R> T;
-        const R fhat = rot_flux<r, R>(wp, wm);
+        const R fhat = rot_flux<r, ORDER, R>(wp, wm, eps);
         const R mdiv = (fhat_prev - fhat) * coef;
         fhat_prev = fhat;
         R o;
@@ -303,7 +343,7 @@ struct SweepCtx {
     }
 };
 
-template <typename R, int DIR, int OUT, int NF>
+template <typename R, int ORDER, int DIR, int OUT, int NF>
 __global__ void __launch_bounds__(32 * NF, ring_blocks_per_sm(NF, sizeof(R)))
 k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
     // 1024-byte alignment: the swizzle pattern is a function of the absolute shared address
@@ -376,7 +416,7 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
         if (nchunks > 1) issue(1);
     }
 
-    SweepCtx<R, DIR, OUT, NF> cx;
+    SweepCtx<R, ORDER, DIR, OUT, NF> cx;
     cx.wp.clear();
     cx.wm.clear();
     cx.fhat_prev = R(0);
@@ -440,7 +480,7 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
             // warm-up chunk: cells s0-4 .. s0+3 fill both windows; the last row gives the interface s0 - 1/2
             cx.template load_push<0>(); cx.template load_push<1>(); cx.template load_push<2>(); cx.template load_push<3>();
             cx.template load_push<4>(); cx.template load_push<5>(); cx.template load_push<6>(); cx.template load_push<7>();
-            cx.fhat_prev = rot_flux<7, R>(cx.wp, cx.wm);
+            cx.fhat_prev = rot_flux<7, ORDER, R>(cx.wp, cx.wm, cx.eps);
         } else {
             cx.template row<0>(); cx.template row<1>(); cx.template row<2>(); cx.template row<3>();
             cx.template row<4>(); cx.template row<5>(); cx.template row<6>(); cx.template row<7>();

@@ -329,6 +329,52 @@ def test_fp32_variant(H, oracle, cfg, n, steps):
     g.close(), o.close()
 
 
+# ------------------------------------------------------------------------------------------------ WENO5 variant (f-2)
+@pytest.mark.parametrize("n", [(32, 32, 32), (37, 19, 23), (7, 5, 3), (130, 9, 6), (64, 40, 72)])
+@pytest.mark.parametrize("nf", [4, 5])
+def test_weno5_rhs_single_stage_parity(H, oracle, n, nf):
+    c = S.scaled_config(0, n)
+    c["nf"] = nf
+    c["jets"] = [((-0.12, 0.03, 0.0), (1.0, 0.5, -0.25))]
+    U0 = S.make_state(c)
+    g = H.Hydro(*n, c["dx"], c["dt"], nfields=nf, weno_order=5)
+    o = oracle.Oracle(*n, c["dx"], c["dt"], nfields=nf, weno_order=5)
+    g.set_state(U0), o.set_state(U0)
+    for pos, d in c["jets"]:
+        g.add_jet(pos, d), o.add_jet(pos, d)
+    for stage_c in (0.0, 0.5):
+        Lg, Lo = g.eval_rhs(stage_c), o.eval_rhs(stage_c)
+        scale = np.max(np.abs(Lo), axis=(1, 2, 3))
+        for f in range(nf):
+            assert np.max(np.abs(Lg[f] - Lo[f])) <= TOL_STAGE * max(scale[f], scale[0]), (f, stage_c)
+    # and it is a different scheme from WENO7
+    g7 = H.Hydro(*n, c["dx"], c["dt"], nfields=nf)
+    g7.set_state(U0)
+    assert np.max(np.abs(g7.eval_rhs(0.0)[0] - g.eval_rhs(0.0)[0])) > 1e-9 * scale[0]
+    g.close(), o.close(), g7.close()
+
+
+@pytest.mark.parametrize("prec,tol", [(64, TOL_RUN), (32, 1e-4)])
+def test_weno5_runs(H, oracle, prec, tol):
+    """WENO5 variant: config 0 (10 steps, jet) and the jet/cap case, fp64 and fp32."""
+    for cfg, n, steps in ((0, (32, 32, 32), 10), (2, (64, 32, 32), 40)):
+        c = S.scaled_config(cfg, n)
+        if cfg == 2:
+            c["jets"] = [((-2.0, 0.0, 0.0), (1.0, 0.0, 0.0))]
+        dt_np = np.float64 if prec == 64 else np.float32
+        U0 = S.make_state(c).astype(dt_np)
+        g = H.Hydro(*n, c["dx"], c["dt"], precision=prec, weno_order=5)
+        o = oracle.Oracle(*n, c["dx"], c["dt"], weno_order=5, v_cap_delta=1e-10 if prec == 64 else 1e-5)
+        g.set_state(U0), o.set_state(U0.astype(np.float64))
+        for pos, d in c["jets"]:
+            g.add_jet(pos, d), o.add_jet(pos, d)
+        g.step(steps), o.step(steps)
+        errs = r13(g.get_fields().astype(np.float64), o.get_fields())
+        assert max(errs) < tol, (cfg, errs)
+        assert g.diag()["has_nan"] == 0
+        g.close(), o.close()
+
+
 # ------------------------------------------------------------------------------------------------ invariants on the GPU
 def test_gpu_uniform_state_and_symmetry(H):
     n = (40, 24, 17)
