@@ -268,6 +268,7 @@ int jet_axis_index(double x, int n, double dx) {
 struct Oracle {
     int nx, ny, nz, nf, order;      // order: 7 (the paper's scheme) or 5 (its WENO5 variant, f-2)
     double dx, dt, eps, delta, e_floor;
+    double sigma;                   // deposit width [fm]; 0 = point deposit (R7), > 0 = Gaussian (R15, f-3)
     long long step;                 // integer step counter; t = step*dt (O1)
     std::vector<double> U, U1, U2, L;
     std::vector<Prim<double> > P;
@@ -363,10 +364,47 @@ void eval_rhs(Oracle& o, const std::vector<double>& U, double stage_c, std::vect
         if (ci >= 0 && cj >= 0 && ck >= 0) {
             size_t c = o.idx(ci, cj, ck);
             q = source_q(o.P[c].e, ell, jt.k_rad, jt.k_coll, jt.crcf);
-            L[c] += q / dx3;
-            L[N + c] += q * jt.nx / dx3;
-            L[2 * N + c] += q * jt.ny / dx3;
-            L[3 * N + c] += q * jt.nz / dx3;
+            if (!(o.sigma > 0.0)) {                  // R7: everything into the one cell
+                L[c] += q / dx3;
+                L[N + c] += q * jt.nx / dx3;
+                L[2 * N + c] += q * jt.ny / dx3;
+                L[3 * N + c] += q * jt.nz / dx3;
+            } else {
+                // R15: delta^3 of eq. (2) -> normalised Gaussian of width sigma around the jet
+                // position, sampled at the centres of the (2R+1)^3 cells around the R7 cell, R = ceil(3 sigma/dx - 2^-20)
+                // (biased like R7 so that 3 sigma = an integer number of cells is not at the mercy of rounding; 1 <= R <= 8); the weights are normalised over the whole cube, so the part that falls outside
+                // the grid is lost through the boundary.  T (hence q) is still taken at the R7 cell.
+                int Rr = (int)std::ceil(3.0 * o.sigma / o.dx - 1.0 / 1048576.0);
+                if (Rr < 1) Rr = 1;
+                if (Rr > 8) Rr = 8;
+                const double xj = jt.x0 + jt.nx * ell, yj = jt.y0 + jt.ny * ell, zj = jt.z0 + jt.nz * ell;
+                const double inv2s2 = 1.0 / (2.0 * o.sigma * o.sigma);
+                // weights relative to the R7 cell (whose centre is the nearest one): w = exp(-(r^2 - r0^2)/(2 sigma^2)),
+                // so that w(R7 cell) = 1 and nothing underflows when sigma << dx
+                const double x0c = (ci + 0.5 - 0.5 * nx) * o.dx - xj, y0c = (cj + 0.5 - 0.5 * ny) * o.dx - yj,
+                             z0c = (ck + 0.5 - 0.5 * nz) * o.dx - zj;
+                const double r02 = x0c * x0c + y0c * y0c + z0c * z0c;
+                double wsum = 0.0;
+                for (int dk = -Rr; dk <= Rr; ++dk) for (int dj = -Rr; dj <= Rr; ++dj) for (int di = -Rr; di <= Rr; ++di) {
+                    double ddx = ((ci + di) + 0.5 - 0.5 * nx) * o.dx - xj;
+                    double ddy = ((cj + dj) + 0.5 - 0.5 * ny) * o.dx - yj;
+                    double ddz = ((ck + dk) + 0.5 - 0.5 * nz) * o.dx - zj;
+                    wsum += std::exp(-((ddx * ddx + ddy * ddy + ddz * ddz) - r02) * inv2s2);
+                }
+                for (int dk = -Rr; dk <= Rr; ++dk) for (int dj = -Rr; dj <= Rr; ++dj) for (int di = -Rr; di <= Rr; ++di) {
+                    int i2 = ci + di, j2 = cj + dj, k2 = ck + dk;
+                    if (i2 < 0 || i2 >= nx || j2 < 0 || j2 >= ny || k2 < 0 || k2 >= nz) continue;
+                    double ddx = (i2 + 0.5 - 0.5 * nx) * o.dx - xj;
+                    double ddy = (j2 + 0.5 - 0.5 * ny) * o.dx - yj;
+                    double ddz = (k2 + 0.5 - 0.5 * nz) * o.dx - zj;
+                    double w = std::exp(-((ddx * ddx + ddy * ddy + ddz * ddz) - r02) * inv2s2) / wsum;
+                    size_t c2 = o.idx(i2, j2, k2);
+                    L[c2] += q * w / dx3;
+                    L[N + c2] += q * w * jt.nx / dx3;
+                    L[2 * N + c2] += q * w * jt.ny / dx3;
+                    L[3 * N + c2] += q * w * jt.nz / dx3;
+                }
+            }
         }
         if (J < 16 && stage_no >= 0) o.last_q[stage_no][J] = q;
     }
@@ -407,7 +445,7 @@ void* oracle_create(int nx, int ny, int nz, double dx, double dt, int nfields, d
     Oracle* o = new Oracle();
     o->nx = nx; o->ny = ny; o->nz = nz; o->nf = nfields; o->dx = dx; o->dt = dt;
     o->eps = weno_eps; o->delta = v_cap_delta; o->e_floor = e_floor;
-    o->step = 0; o->ncap = 0; o->has_nan = 0; o->order = 7;
+    o->step = 0; o->ncap = 0; o->has_nan = 0; o->order = 7; o->sigma = 0.0;
     size_t T = o->N() * nfields;
     o->U.assign(T, 0.0); o->U1.assign(T, 0.0); o->U2.assign(T, 0.0); o->L.assign(T, 0.0);
     o->P.resize(o->N());
@@ -417,6 +455,12 @@ void* oracle_create(int nx, int ny, int nz, double dx, double dt, int nfields, d
     return o;
 }
 void oracle_destroy(void* h) { delete (Oracle*)h; }
+// width of the Gaussian deposit [fm] (R15, f-3); 0 restores the point deposit of R7
+int oracle_set_deposit_width(void* h, double sigma) {
+    if (!(sigma >= 0.0)) return 1;
+    ((Oracle*)h)->sigma = sigma;
+    return 0;
+}
 // spatial order of the reconstruction: 7 (default, "currently we use") or 5 (f-2); returns 0 on success
 int oracle_set_weno_order(void* h, int order) {
     if (order != 5 && order != 7) return 1;

@@ -59,6 +59,8 @@ def lib():
         L.oracle_weno7_parts.argtypes = [dp, d, dp, dp, dp, dp]
         L.oracle_interface_flux.argtypes = [i, i, dp, d, d, d, d, dp]
         L.oracle_interface_flux_order.argtypes = [i, i, dp, d, d, d, d, i, dp]
+        L.oracle_set_deposit_width.restype = i
+        L.oracle_set_deposit_width.argtypes = [p, d]
         L.oracle_set_weno_order.restype = i
         L.oracle_set_weno_order.argtypes = [p, i]
         L.oracle_weno5.restype = d
@@ -124,6 +126,11 @@ class Oracle:
     def clear_jets(self):
         self.L.oracle_clear_jets(self.h)
         self.njets = 0
+
+    def set_deposit_width(self, sigma):
+        """Gaussian deposit of width sigma [fm] (reading R15); 0 = point deposit (R7)."""
+        if self.L.oracle_set_deposit_width(self.h, float(sigma)):
+            raise ValueError("sigma must be >= 0")
 
     def step(self, n=1):
         self.L.oracle_step(self.h, int(n))

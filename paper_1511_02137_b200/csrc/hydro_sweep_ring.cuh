@@ -96,8 +96,9 @@ __host__ __device__ constexpr int ring_smem_bytes(int nf, int out, int esz) {
            + 64;                                           // mbarriers
 }
 // resident blocks per SM the kernels are compiled for (registers: 65536 / (32 NF threads x blocks))
-__host__ __device__ constexpr int ring_blocks_per_sm(int nf, int esz) {
-    return esz == 8 ? (nf == 4 ? 3 : 2) : (nf == 4 ? 5 : 4);
+__host__ __device__ constexpr int ring_blocks_per_sm(int nf, int esz, int out = OUT_COMBINE) {
+    // nf = 5 in fp64: 3 blocks (<= 136 registers, 64 KB) except the combine kernel with its U^n tiles (84 KB): 2
+    return esz == 8 ? (nf == 4 ? 3 : (out != OUT_COMBINE ? 3 : 2)) : (nf == 4 ? 5 : 4);
 }
 
 struct RingMaps {
@@ -344,7 +345,7 @@ struct SweepCtx {
 };
 
 template <typename R, int ORDER, int DIR, int OUT, int NF>
-__global__ void __launch_bounds__(32 * NF, ring_blocks_per_sm(NF, sizeof(R)))
+__global__ void __launch_bounds__(32 * NF, ring_blocks_per_sm(NF, sizeof(R), OUT))
 k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
     // 1024-byte alignment: the swizzle pattern is a function of the absolute shared address
     extern __shared__ __align__(1024) unsigned char smem[];
