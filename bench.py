@@ -116,7 +116,7 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_slab_run(cfg, nzs, steps, warmup=0, order=7):
+def oracle_slab_run(cfg, nzs, steps, warmup=0, order=7, sigma=0.0):
     """Oracle on the central nzs planes of config `cfg`'s initial condition; returns (cells, seconds, threads)."""
     from oracle import oracle as O
     c = S.CONFIGS[cfg]
@@ -127,6 +127,7 @@ def oracle_slab_run(cfg, nzs, steps, warmup=0, order=7):
     o.set_state(U0)
     for pos, d in c["jets"]:
         o.add_jet(pos, d, S.KAPPA_RAD, S.KAPPA_COLL, S.CR_OVER_CF)
+    o.set_deposit_width(sigma)
     if warmup:
         o.step(warmup)
     t0 = time.perf_counter()
@@ -143,10 +144,10 @@ def run_reference(args, rank):
     cfg = args.config
     c = S.CONFIGS[cfg]
     # size the slab so that (K + W) steps take about two minutes: calibrate on one step of 8 planes
-    cells8, t8, threads = oracle_slab_run(cfg, 8, 1, order=args.weno_order)
+    cells8, t8, threads = oracle_slab_run(cfg, 8, 1, order=args.weno_order, sigma=args.deposit_sigma)
     budget = 120.0
     nzs = int(min(c["n"][2], max(8, 8 * int(budget / (t8 * (args.steps + args.warmup)) + 1e-9))))
-    cells, secs, threads = oracle_slab_run(cfg, nzs, args.steps, args.warmup, order=args.weno_order)
+    cells, secs, threads = oracle_slab_run(cfg, nzs, args.steps, args.warmup, order=args.weno_order, sigma=args.deposit_sigma)
     value = cells * args.steps / secs
     sample = "%dx%dx%d central slab of config %d's IC + jet, %d RK3 steps" % (c["n"][0], c["n"][1], nzs, cfg,
                                                                               args.steps)
@@ -166,7 +167,7 @@ def workload_config(args, cfg):
     return {"workload": "BASELINE config %d: %dx%dx%d, dx=%g fm, dt=%g fm/c, nf=%d, p=e/3, ellipsoidal flow + %d jet(s), "
                         "outflow ghosts" % (cfg, c["n"][0], c["n"][1], c["n"][2], c["dx"], c["dt"], c["nf"],
                                             len(c["jets"])),
-            "cells": int(np.prod(c["n"])), "config_steps": c["steps"], "weno_order": getattr(args, "weno_order", 7),
+            "cells": int(np.prod(c["n"])), "config_steps": c["steps"], "weno_order": getattr(args, "weno_order", 7), "deposit_sigma_fm": getattr(args, "deposit_sigma", 0.0),
             "parallelism": "replicas x%d" % args.gpus,
             "l2": "state (%.0f MiB per copy) exceeds L2; no flush needed" %
                   (np.prod(c["n"]) * c["nf"] * (args.precision // 8) / 2 ** 20)}
@@ -181,6 +182,7 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
     ap.add_argument("--weno-order", type=int, default=7, choices=[7, 5])
+    ap.add_argument("--deposit-sigma", type=float, default=0.0, help="Gaussian deposit width [fm] (R15); 0 = one cell")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -220,9 +222,11 @@ def main():
         U0d = U0h.cuda(non_blocking=True)
     stream.synchronize()
     g = H.Hydro(*c["n"], c["dx"], c["dt"], nfields=c["nf"], precision=args.precision, stream=stream,
-                weno_order=args.weno_order)
+                weno_order=args.weno_order, sigma=args.deposit_sigma)
     for pos, d in c["jets"]:
         g.add_jet(pos, d, S.KAPPA_RAD, S.KAPPA_COLL, S.CR_OVER_CF)
+
+    g.set_deposit_width(args.deposit_sigma)
 
     # ---- measured ALU peak of this GPU, same run
     peak_tf = H.measure_alu_peak(args.precision, 200.0, stream.cuda_stream)
@@ -310,7 +314,7 @@ def main():
                            "what": "hydro_set_state(host) + hydro_step(K) + hydro_get_fields(host), pinned buffers; "
                                    "bytes are the one upload / one download spread over K steps"}
         if not args.no_cpu_baseline and world == 1:
-            cells_s, secs, threads = oracle_slab_run(cfg, 16, 2, order=args.weno_order)
+            cells_s, secs, threads = oracle_slab_run(cfg, 16, 2, order=args.weno_order, sigma=args.deposit_sigma)
             line["cpu_baseline"] = {"value": cells_s * 2 / secs, "unit": UNIT, "cores": threads, "kind": "oracle",
                                     "sample": "%dx%dx16 central slab of config %d's IC + jet, 2 RK3 steps (%.1f s)" %
                                               (c["n"][0], c["n"][1], cfg, secs)}

@@ -74,6 +74,10 @@ int hydro_set_state(hydro_t *h, const void *U, int memspace);
 int hydro_add_jet(hydro_t *h, double x0, double y0, double z0, double dirx, double diry, double dirz,
                   double kappa_rad, double kappa_coll, double cr_over_cf, int *id);
 int hydro_clear_jets(hydro_t *h);
+/* Width sigma >= 0 [fm] of the jets' deposit (all jets of the handle).  0 (default): the delta function of eq. (2) is one
+ * cell (R7).  > 0: a normalised Gaussian of that width around the jet position, sampled on the (2R+1)^3 cells around
+ * the R7 cell, R = ceil(3 sigma/dx) clamped to [1, 8] (reading R15). */
+int hydro_set_deposit_width(hydro_t *h, double sigma);
 
 /* Advance nsteps >= 0 full SSP-RK3 steps of size dt: per stage con2prim + wavespeed max (a-1, a-2), the three
  * WENO7 Lax-Friedrichs sweeps (a-3, a-4), the jet source (a-5) and the stage combination (a-6), with

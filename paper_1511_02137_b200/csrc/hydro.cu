@@ -21,6 +21,7 @@ struct hydro {
     int nxp;                            // row pitch in reals: nx rounded up so that a row is a multiple of 16 bytes (TMA)
     long long N, Np;                    // interior cells; field stride nxp*ny*nz
     double dx, dt, weno_eps, delta, e_floor;
+    double sigma;                       // Gaussian deposit width [fm]; 0 = point deposit
     size_t esz;                         // bytes per real
     cudaStream_t stream;
     bool own_stream;
@@ -256,10 +257,10 @@ int launch_source(hydro* h, int slot, int stage, double stage_c, bool commit, do
     SourceArgs s;
     s.diag = h->diag; s.jets = h->jets_dev; s.njets = (int)h->jets.size(); s.slot = slot; s.stage = stage;
     s.commit = commit ? 1 : 0; s.nx = h->nx; s.ny = h->ny; s.nz = h->nz; s.nxp = h->nxp; s.N = h->Np; s.step = h->step;
-    s.stage_c = stage_c; s.dx = h->dx; s.dt = h->dt; s.rk_weight = rk_weight; s.scale = scale;
+    s.stage_c = stage_c; s.dx = h->dx; s.dt = h->dt; s.rk_weight = rk_weight; s.scale = scale; s.sigma = h->sigma;
     {
         Timer t(h, HYDRO_K_SOURCE);
-        k_source<R><<<1, 32, 0, h->stream>>>(s, (const R*)h->P, (R*)target);
+        k_source<R><<<1, SOURCE_THREADS, 0, h->stream>>>(s, (const R*)h->P, (R*)target);
     }
     h->launches += 1;
     CK(cudaGetLastError());
@@ -380,6 +381,7 @@ int hydro_create(hydro_t** out, int nx, int ny, int nz, double dx, double dt, co
     h->nx = nx; h->ny = ny; h->nz = nz; h->nf = o.nfields; h->prec = o.precision;
     h->N = (long long)nx * ny * nz;
     h->order = o.weno_order == 5 ? 5 : 7;
+    h->sigma = 0.0;
     h->dx = dx; h->dt = dt;
     h->weno_eps = o.weno_eps > 0 ? o.weno_eps : 1e-6;
     h->delta = o.v_cap_delta > 0 ? o.v_cap_delta : (o.precision == 64 ? 1e-10 : 1e-5);
@@ -472,6 +474,12 @@ int hydro_add_jet(hydro_t* h, double x0, double y0, double z0, double dirx, doub
     h->jets.push_back(j);
     h->jets_dirty = true;
     if (id) *id = (int)h->jets.size() - 1;
+    return HYDRO_OK;
+}
+
+int hydro_set_deposit_width(hydro_t* h, double sigma) {
+    if (!h || !(sigma >= 0.0) || !std::isfinite(sigma)) return HYDRO_EINVAL;
+    h->sigma = sigma;
     return HYDRO_OK;
 }
 

@@ -263,6 +263,7 @@ struct SourceArgs {
     long long N /* field stride Np */, step;
     double stage_c, dx, dt, rk_weight;
     double scale;                      // the deposit is added to `target` times this (1 for L, b dt for a stage state)
+    double sigma;                      // Gaussian deposit width [fm] (R15); 0 = point deposit (R7)
 };
 
 __device__ __forceinline__ int jet_axis_index(double x, int n, double dx) {
@@ -273,47 +274,108 @@ __device__ __forceinline__ int jet_axis_index(double x, int n, double dx) {
     return (int)fl;
 }
 
+constexpr int SOURCE_THREADS = 256;
+
+// One block.  Thread 0 does the bookkeeping and the point deposit (R7); with sigma > 0 (reading R15)
+// the whole block spreads q over the (2R+1)^3 cells around the R7 cell with normalised Gaussian weights
+// w = exp(-(r^2 - r0^2) / (2 sigma^2)) (r: cell centre to jet position, r0: that of the R7 cell), R = ceil(3 sigma/dx -
+// 2^-20) in [1, 8]; the sum of the weights is reduced in a fixed order (bitwise reproducible); the part of the cube
+// outside the grid is lost.  Jets are processed one after the other, so overlapping deposits add in a fixed order.
 template <typename R>
-__global__ void k_source(SourceArgs a, const R* __restrict__ P, R* __restrict__ L /* target */) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+__global__ void __launch_bounds__(SOURCE_THREADS) k_source(SourceArgs a, const R* __restrict__ P, R* __restrict__ L /* target */) {
+    __shared__ double sh_q, sh_pos[3], sh_red[SOURCE_THREADS];
+    __shared__ int sh_c[3];
+    const int tid = threadIdx.x;
     Diag* dg = a.diag;
-    const DiagSlot* s = &dg->slot[a.slot];
+    if (tid == 0) {
+        const DiagSlot* s = &dg->slot[a.slot];
 #pragma unroll
-    for (int d = 0; d < 3; ++d) dg->alpha_last[d] = (double)Real<R>::from_bits(s->alpha_bits[d]);
-    if (a.commit) {
-        dg->ncap_total += s->ncap;
-        dg->nan_total |= s->nan_flag;
+        for (int d = 0; d < 3; ++d) dg->alpha_last[d] = (double)Real<R>::from_bits(s->alpha_bits[d]);
+        if (a.commit) {
+            dg->ncap_total += s->ncap;
+            dg->nan_total |= s->nan_flag;
+        }
     }
     const double HBARC = 0.1973269804;
     const double G_DOF = 47.5 * 3.14159265358979323846 * 3.14159265358979323846 / 30.0;
     const double dx3 = a.dx * a.dx * a.dx;
     for (int J = 0; J < a.njets; ++J) {
         const JetDev jt = a.jets[J];
-        const double ell = __dmul_rn(__dadd_rn((double)(a.step - jt.step_added), a.stage_c), a.dt);
-        const int ci = jet_axis_index(__dadd_rn(jt.x0, __dmul_rn(jt.nx, ell)), a.nx, a.dx);
-        const int cj = jet_axis_index(__dadd_rn(jt.y0, __dmul_rn(jt.ny, ell)), a.ny, a.dx);
-        const int ck = jet_axis_index(__dadd_rn(jt.z0, __dmul_rn(jt.nz, ell)), a.nz, a.dx);
-        double q = 0.0;
-        if (ci >= 0 && cj >= 0 && ck >= 0) {
-            const long long c = ((long long)ck * a.ny + cj) * a.nxp + ci;
-            const double e_c = 3.0 * (double)P[c];
-            const double T2 = sqrt(e_c / (G_DOF * HBARC));       // T^2, T in 1/fm
-            const double T = sqrt(T2);
-            q = HBARC * jt.crcf * (jt.k_rad * T2 * T * ell + jt.k_coll * T2);
-            const double r = a.scale * (q / dx3);
-            L[c] += (R)r;
-            L[a.N + c] += (R)(r * jt.nx);
-            L[2 * a.N + c] += (R)(r * jt.ny);
-            L[3 * a.N + c] += (R)(r * jt.nz);
+        if (tid == 0) {
+            const double ell = __dmul_rn(__dadd_rn((double)(a.step - jt.step_added), a.stage_c), a.dt);
+            const double xj = __dadd_rn(jt.x0, __dmul_rn(jt.nx, ell)), yj = __dadd_rn(jt.y0, __dmul_rn(jt.ny, ell)),
+                         zj = __dadd_rn(jt.z0, __dmul_rn(jt.nz, ell));
+            const int ci = jet_axis_index(xj, a.nx, a.dx);
+            const int cj = jet_axis_index(yj, a.ny, a.dx);
+            const int ck = jet_axis_index(zj, a.nz, a.dx);
+            double q = 0.0;
+            if (ci >= 0 && cj >= 0 && ck >= 0) {
+                const long long c = ((long long)ck * a.ny + cj) * a.nxp + ci;
+                const double e_c = 3.0 * (double)P[c];
+                const double T2 = sqrt(e_c / (G_DOF * HBARC));       // T^2, T in 1/fm
+                const double T = sqrt(T2);
+                q = HBARC * jt.crcf * (jt.k_rad * T2 * T * ell + jt.k_coll * T2);
+                if (!(a.sigma > 0.0)) {
+                    const double r = a.scale * (q / dx3);
+                    L[c] += (R)r;
+                    L[a.N + c] += (R)(r * jt.nx);
+                    L[2 * a.N + c] += (R)(r * jt.ny);
+                    L[3 * a.N + c] += (R)(r * jt.nz);
+                }
+            }
+            if (a.commit) {
+                if (J < MAX_JETS) dg->last_q[a.stage][J] = q;
+                const double amt = a.dt * a.rk_weight * q;
+                dg->deposited[0] += amt;
+                dg->deposited[1] += amt * jt.nx;
+                dg->deposited[2] += amt * jt.ny;
+                dg->deposited[3] += amt * jt.nz;
+            }
+            sh_q = q; sh_pos[0] = xj; sh_pos[1] = yj; sh_pos[2] = zj;
+            sh_c[0] = ci; sh_c[1] = cj; sh_c[2] = ck;
         }
-        if (a.commit) {
-            if (J < MAX_JETS) dg->last_q[a.stage][J] = q;
-            const double amt = a.dt * a.rk_weight * q;
-            dg->deposited[0] += amt;
-            dg->deposited[1] += amt * jt.nx;
-            dg->deposited[2] += amt * jt.ny;
-            dg->deposited[3] += amt * jt.nz;
+        if (!(a.sigma > 0.0)) continue;                              // uniform: no barrier needed for the point deposit
+        __syncthreads();
+        const int ci = sh_c[0], cj = sh_c[1], ck = sh_c[2];
+        const double q = sh_q;
+        if (ci >= 0 && cj >= 0 && ck >= 0) {                         // uniform across the block
+            int Rr = (int)ceil(__dadd_rn(__ddiv_rn(__dmul_rn(3.0, a.sigma), a.dx), -1.0 / 1048576.0));
+            Rr = Rr < 1 ? 1 : (Rr > 8 ? 8 : Rr);
+            const int side = 2 * Rr + 1, ncell = side * side * side;
+            const double inv2s2 = 1.0 / (2.0 * a.sigma * a.sigma);
+            const double x0c = ((ci + 0.5) - 0.5 * a.nx) * a.dx - sh_pos[0], y0c = ((cj + 0.5) - 0.5 * a.ny) * a.dx - sh_pos[1],
+                         z0c = ((ck + 0.5) - 0.5 * a.nz) * a.dx - sh_pos[2];
+            const double r02 = x0c * x0c + y0c * y0c + z0c * z0c;
+            auto weight = [&](int s, int& i2, int& j2, int& k2) {
+                const int di = s % side - Rr, dj = (s / side) % side - Rr, dk = s / (side * side) - Rr;
+                i2 = ci + di; j2 = cj + dj; k2 = ck + dk;
+                const double ddx = ((i2 + 0.5) - 0.5 * a.nx) * a.dx - sh_pos[0];
+                const double ddy = ((j2 + 0.5) - 0.5 * a.ny) * a.dx - sh_pos[1];
+                const double ddz = ((k2 + 0.5) - 0.5 * a.nz) * a.dx - sh_pos[2];
+                return exp(-((ddx * ddx + ddy * ddy + ddz * ddz) - r02) * inv2s2);
+            };
+            double part = 0.0;
+            int i2, j2, k2;
+            for (int s = tid; s < ncell; s += SOURCE_THREADS) part += weight(s, i2, j2, k2);
+            sh_red[tid] = part;
+            __syncthreads();
+            for (int off = SOURCE_THREADS / 2; off > 0; off >>= 1) {
+                if (tid < off) sh_red[tid] += sh_red[tid + off];
+                __syncthreads();
+            }
+            const double norm = a.scale * q / (sh_red[0] * dx3);
+            for (int s = tid; s < ncell; s += SOURCE_THREADS) {
+                const double w = weight(s, i2, j2, k2);
+                if (i2 < 0 || i2 >= a.nx || j2 < 0 || j2 >= a.ny || k2 < 0 || k2 >= a.nz) continue;
+                const long long c = ((long long)k2 * a.ny + j2) * a.nxp + i2;
+                const double r = norm * w;
+                L[c] += (R)r;
+                L[a.N + c] += (R)(r * jt.nx);
+                L[2 * a.N + c] += (R)(r * jt.ny);
+                L[3 * a.N + c] += (R)(r * jt.nz);
+            }
         }
+        __syncthreads();                                             // the next jet may touch the same cells / shared slots
     }
 }
 

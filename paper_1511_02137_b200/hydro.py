@@ -22,7 +22,7 @@ FIELDS_CONSERVED, FIELDS_PRIMITIVE = 0, 1
 K_NAMES = ("prim", "sweep_x", "sweep_y", "sweep_z", "source")
 
 # every symbol include/hydro.h declares (tests check that the library exports all of them)
-SYMBOLS = ("hydro_create", "hydro_destroy", "hydro_set_state", "hydro_add_jet", "hydro_clear_jets", "hydro_step",
+SYMBOLS = ("hydro_create", "hydro_destroy", "hydro_set_state", "hydro_add_jet", "hydro_clear_jets", "hydro_set_deposit_width", "hydro_step",
            "hydro_synchronize", "hydro_get_fields", "hydro_eval_rhs", "hydro_get_diag", "hydro_get_last_stage_q",
            "hydro_set_profiling", "hydro_get_kernel_times", "hydro_launch_count", "hydro_sweep_path", "hydro_measure_alu_peak",
            "hydro_strerror", "hydro_last_cuda_error")
@@ -63,6 +63,8 @@ def load():
     L.hydro_add_jet.argtypes = [vp] + [d] * 9 + [C.POINTER(i)]
     L.hydro_clear_jets.restype = i
     L.hydro_clear_jets.argtypes = [vp]
+    L.hydro_set_deposit_width.restype = i
+    L.hydro_set_deposit_width.argtypes = [vp, d]
     L.hydro_step.restype = i
     L.hydro_step.argtypes = [vp, i]
     L.hydro_synchronize.restype = i
@@ -180,6 +182,9 @@ class Hydro:
     def clear_jets(self):
         self._ck(self.L.hydro_clear_jets(self.h), "hydro_clear_jets")
         self.njets = 0
+
+    def set_deposit_width(self, sigma):
+        self._ck(self.L.hydro_set_deposit_width(self.h, float(sigma)), "hydro_set_deposit_width")
 
     def step(self, n=1):
         self._ck(self.L.hydro_step(self.h, int(n)), "hydro_step")

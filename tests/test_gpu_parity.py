@@ -375,6 +375,50 @@ def test_weno5_runs(H, oracle, prec, tol):
         g.close(), o.close()
 
 
+# ------------------------------------------------------------------------------------------------ smeared deposit (f-3)
+@pytest.mark.parametrize("sigma", [0.05, 0.1, 0.25])
+def test_smeared_deposit_rhs_parity(H, oracle, sigma):
+    """Reading R15: the Gaussian deposit of several jets (one near a corner, one outside the grid) on the GPU and in
+    the oracle: same support (integer work) and the same values."""
+    c = S.scaled_config(0, (26, 21, 16))
+    c["jets"] = [((0.0, 0.0, 0.0), (1.0, 0.0, 0.0)), ((0.02, 0.01, 0.0), (-1.0, 0.0, 0.0)),
+                 ((-0.35, 0.25, 0.05), (0.3, -0.4, 0.2)), ((1.25, 1.0, 0.75), (1.0, 1.0, 1.0)), ((9.0, 0.0, 0.0), (1.0, 0.0, 0.0))]
+    for stage_c in (0.0, 0.5):
+        _, U0, g, o = make_pair(H, oracle, c)
+        _, _, g0, o0 = make_pair(H, oracle, c, jets=False)
+        g.set_deposit_width(sigma), o.set_deposit_width(sigma)
+        dLg = g.eval_rhs(stage_c) - g0.eval_rhs(stage_c)
+        dLo = o.eval_rhs(stage_c) - o0.eval_rhs(stage_c)
+        big = np.abs(dLo) > 1e-9 * np.max(np.abs(dLo))            # tiny tails may round to the background's ulp
+        assert np.array_equal((dLg != 0)[big], (dLo != 0)[big])
+        assert np.max(np.abs(dLg - dLo)) < 1e-11 * np.max(np.abs(dLo))
+        for x in (g, o, g0, o0):
+            x.close()
+
+
+@pytest.mark.parametrize("prec,tol", [(64, TOL_RUN), (32, 1e-4)])
+def test_smeared_deposit_run(H, oracle, prec, tol):
+    """The jet/cap case of test_jet_run_with_cap_events with a Gaussian deposit of width dx: parity after the run, the
+    deposited totals agree, and (SURVEY f-3) the smearing removes the cap events the point deposit causes."""
+    c = S.scaled_config(2, (64, 32, 32))
+    c["jets"] = [((-2.0, 0.0, 0.0), (1.0, 0.0, 0.0)), ((2.0, 0.5, 0.0), (-1.0, 0.0, 0.0))]
+    steps = 40
+    U0 = S.make_state(c).astype(np.float64 if prec == 64 else np.float32)
+    g = H.Hydro(*c["n"], c["dx"], c["dt"], precision=prec)
+    o = oracle.Oracle(*c["n"], c["dx"], c["dt"], v_cap_delta=1e-10 if prec == 64 else 1e-5)
+    g.set_state(U0), o.set_state(U0.astype(np.float64))
+    for pos, d in c["jets"]:
+        g.add_jet(pos, d), o.add_jet(pos, d)
+    g.set_deposit_width(0.1), o.set_deposit_width(0.1)
+    g.step(steps), o.step(steps)
+    errs = r13(g.get_fields().astype(np.float64), o.get_fields())
+    assert max(errs) < tol, errs
+    dg, do = g.diag(), o.diag()
+    assert np.max(np.abs(dg["deposited"] - do["deposited"])) <= (1e-10 if prec == 64 else 1e-4) * do["deposited"][0]
+    assert dg["has_nan"] == 0 and dg["ncap"] == do["ncap"] == 0
+    g.close(), o.close()
+
+
 # ------------------------------------------------------------------------------------------------ invariants on the GPU
 def test_gpu_uniform_state_and_symmetry(H):
     n = (40, 24, 17)
