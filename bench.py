@@ -222,7 +222,7 @@ def main():
         U0d = U0h.cuda(non_blocking=True)
     stream.synchronize()
     g = H.Hydro(*c["n"], c["dx"], c["dt"], nfields=c["nf"], precision=args.precision, stream=stream,
-                weno_order=args.weno_order, sigma=args.deposit_sigma)
+                weno_order=args.weno_order)
     for pos, d in c["jets"]:
         g.add_jet(pos, d, S.KAPPA_RAD, S.KAPPA_COLL, S.CR_OVER_CF)
 
