@@ -95,13 +95,16 @@ __host__ __device__ constexpr int ring_smem_bytes(int nf, int out, int esz) {
             + RING_SUB) * esz                              // one tile of zeros
            + 64;                                           // mbarriers
 }
+#ifndef RING_F64_BLOCKS
+#define RING_F64_BLOCKS 3
+#endif
 #ifndef RING_F32_BLOCKS
 #define RING_F32_BLOCKS 6
 #endif
 // resident blocks per SM the kernels are compiled for (registers: 65536 / (32 NF threads x blocks))
 __host__ __device__ constexpr int ring_blocks_per_sm(int nf, int esz, int out = OUT_COMBINE) {
     // nf = 5 in fp64: 3 blocks (<= 136 registers, 64 KB) except the combine kernel with its U^n tiles (84 KB): 2
-    return esz == 8 ? (nf == 4 ? 3 : (out != OUT_COMBINE ? 3 : 2)) : (nf == 4 ? RING_F32_BLOCKS : 4);
+    return esz == 8 ? (nf == 4 ? RING_F64_BLOCKS : (out != OUT_COMBINE ? 3 : 2)) : (nf == 4 ? RING_F32_BLOCKS : 4);
 }
 
 struct RingMaps {

@@ -329,6 +329,36 @@ def test_fp32_variant(H, oracle, cfg, n, steps):
     g.close(), o.close()
 
 
+def test_config4_full_size_properties(H):
+    """BASELINE config 4 at its full size (512^3, nf = 5, two back-to-back jets; 22 GiB on the device), a few steps on
+    the GPU alone (the oracle would need ~30 GB and minutes): properties that hold at any size -- finite state, both
+    jets start in the same cell with opposite directions so the deposited momentum cancels at l = 0 and stays well
+    below the deposited energy (the +x jet stays in the cell both heated, so its q is somewhat larger), the baryon number only changes through the boundary, a repeated run is bitwise equal."""
+    import torch
+    if torch.cuda.mem_get_info()[1] < 40 * 2 ** 30:
+        pytest.skip("needs a device with > 40 GiB")
+    c = S.CONFIGS[4]
+    steps = int(os.environ.get("HYDRO_TEST_CFG4_STEPS", "2"))
+    U0 = S.make_state(4)
+    g = H.Hydro(*c["n"], c["dx"], c["dt"], nfields=5)
+    g.set_state(U0)
+    for pos, d in c["jets"]:
+        g.add_jet(pos, d)
+    g.step(steps)
+    U = g.get_fields()
+    dg = g.diag()
+    assert dg["has_nan"] == 0 and dg["step"] == steps and np.all(np.isfinite(U[:, ::7, ::5, ::3]))
+    q = g.last_stage_q()
+    assert q.shape == (3, 2) and np.all(q > 0)
+    assert dg["deposited"][0] > 0 and abs(dg["deposited"][1]) < 0.5 * dg["deposited"][0]
+    nb0, nb1 = U0[4].sum(dtype=np.longdouble), U[4].sum(dtype=np.longdouble)
+    assert abs(float(nb1 - nb0)) < 1e-3 * float(nb0)                      # only boundary outflow of the 0.01 background
+    g.set_state(U0)
+    g.step(steps)
+    assert np.array_equal(g.get_fields()[:, 250:262], U[:, 250:262])
+    g.close()
+
+
 # ------------------------------------------------------------------------------------------------ WENO5 variant (f-2)
 @pytest.mark.parametrize("n", [(32, 32, 32), (37, 19, 23), (7, 5, 3), (130, 9, 6), (64, 40, 72)])
 @pytest.mark.parametrize("nf", [4, 5])
