@@ -269,6 +269,8 @@ struct Oracle {
     int nx, ny, nz, nf, order;      // order: 7 (the paper's scheme) or 5 (its WENO5 variant, f-2)
     double dx, dt, eps, delta, e_floor;
     double sigma;                   // deposit width [fm]; 0 = point deposit (R7), > 0 = Gaussian (R15, f-3)
+    int limiter;                    // 1: positivity-preserving flux limiter (R16, f-1)
+    long long nlim;                 // faces limited (theta < 1), cumulative over stages
     long long step;                 // integer step counter; t = step*dt (O1)
     std::vector<double> U, U1, U2, L;
     std::vector<Prim<double> > P;
@@ -281,6 +283,117 @@ struct Oracle {
     size_t N() const { return (size_t)nx * ny * nz; }
     size_t idx(int i, int j, int k) const { return ((size_t)k * ny + j) * nx + i; }
 };
+
+// ---------------------------------------------------------------- f-1: positivity-preserving flux limiter
+// SURVEY 8(f) f-1; PAPER.md:25 cites the positivity-preserving FD-WENO paper [2] (:58) but gives no detail, so this is
+// reading R16, built from the concavity of g(U) = E - |M| (g > 0 <=> e > 0 for p = e/3):
+//   * every interface flux is  F^L + theta C,  F^L = f+_i + f-_{i+1} = (F_i + F_{i+1})/2 - alpha (U_{i+1} - U_i)/2 the
+//     first-order Lax-Friedrichs flux, C = F^H - F^L the high-order (WENO) correction, one theta in [0,1] per face;
+//   * U^L = U - (dt/dx) sum_faces +-F^L (the first-order update) is admissible for 3 alpha dt/dx <= 1 (convex
+//     combination of U and U -+ F/alpha states; the paper's dt/dx = 0.2 qualifies);
+//   * the limited update is the average of the six states  W_f = U^L_i -+ 6 (dt/dx) theta_f C_f,  so it is admissible
+//     if every W_f is: theta_f = min over the two cells of the face of
+//         1                                   if g(W_f(1)) >= delta_i
+//         (g(U^L_i) - delta_i) / (g(U^L_i) - g(W_f(1)))   otherwise   (g concave => g(W_f(theta)) >= delta_i),
+//     delta_i = min(1e-8 E^L_i, g(U^L_i));  ghost cells impose no condition;
+//   * the jet deposit is light-like (g = 0) and g is superadditive, so adding dt S afterwards keeps g >= delta;
+//   * SSP-RK3 stages are convex combinations of such Euler steps.  The baryon density uses the same theta.
+// Output: L -= divergence of the limited fluxes (so that U + dt L is the limited Euler update); counts faces with theta < 1.
+inline double g_adm(const double W[4]) { return W[0] - std::sqrt(W[1] * W[1] + W[2] * W[2] + W[3] * W[3]); }
+
+void limited_divergence(Oracle& o, const std::vector<double>& U, std::vector<double>& L) {
+    const int nx = o.nx, ny = o.ny, nz = o.nz, nf = o.nf;
+    const size_t N = o.N();
+    const double lam = o.dt / o.dx;
+    std::vector<double> FL[3], CC[3], TH[3];
+    std::vector<double> UL(U.begin(), U.end());
+    for (int d = 0; d < 3; ++d) {
+        const int nd = d == 0 ? nx : d == 1 ? ny : nz, na = d == 0 ? ny : nx, nb = d == 2 ? ny : nz;
+        const double alpha = o.alpha[d];
+        FL[d].assign((size_t)(nd + 1) * na * nb * 5, 0.0);
+        CC[d].assign((size_t)(nd + 1) * na * nb * 5, 0.0);
+        TH[d].assign((size_t)(nd + 1) * na * nb, 1.0);
+#pragma omp parallel for collapse(2)
+        for (int tb = 0; tb < nb; ++tb)
+            for (int ta = 0; ta < na; ++ta)
+                for (int i = -1; i < nd; ++i) {
+                    double Uw[8][5]; Prim<double> Pw[8];
+                    for (int m = 0; m < 8; ++m) {
+                        int sidx = std::min(std::max(i - 3 + m, 0), nd - 1);
+                        size_t c = d == 0 ? o.idx(sidx, ta, tb) : d == 1 ? o.idx(ta, sidx, tb) : o.idx(ta, tb, sidx);
+                        for (int q = 0; q < nf; ++q) Uw[m][q] = U[q * N + c];
+                        Pw[m] = o.P[c];
+                    }
+                    double FH[5], Fi[5], Fj[5];
+                    interface_flux<double>(d, nf, Uw, Pw, alpha, o.eps, FH, o.order);
+                    phys_flux<double>(d, Uw[3], Pw[3], nf, Fi);          // cell i
+                    phys_flux<double>(d, Uw[4], Pw[4], nf, Fj);          // cell i+1
+                    const size_t f = ((size_t)tb * na + ta) * (nd + 1) + (i + 1);
+                    for (int q = 0; q < nf; ++q) {
+                        double fl = 0.5 * (Fi[q] + alpha * Uw[3][q]) + 0.5 * (Fj[q] - alpha * Uw[4][q]);
+                        FL[d][f * 5 + q] = fl;
+                        CC[d][f * 5 + q] = FH[q] - fl;
+                    }
+                }
+        // first-order update
+#pragma omp parallel for collapse(2)
+        for (int tb = 0; tb < nb; ++tb)
+            for (int ta = 0; ta < na; ++ta)
+                for (int i = 0; i < nd; ++i) {
+                    size_t c = d == 0 ? o.idx(i, ta, tb) : d == 1 ? o.idx(ta, i, tb) : o.idx(ta, tb, i);
+                    const size_t f = ((size_t)tb * na + ta) * (nd + 1) + i;
+                    for (int q = 0; q < nf; ++q) UL[q * N + c] -= lam * (FL[d][(f + 1) * 5 + q] - FL[d][f * 5 + q]);
+                }
+    }
+    // theta per face from the two adjacent cells
+    long long nlim = 0;
+    for (int d = 0; d < 3; ++d) {
+        const int nd = d == 0 ? nx : d == 1 ? ny : nz, na = d == 0 ? ny : nx, nb = d == 2 ? ny : nz;
+#pragma omp parallel for collapse(2) reduction(+ : nlim)
+        for (int tb = 0; tb < nb; ++tb)
+            for (int ta = 0; ta < na; ++ta)
+                for (int i = -1; i < nd; ++i) {
+                    const size_t f = ((size_t)tb * na + ta) * (nd + 1) + (i + 1);
+                    double th = 1.0;
+                    for (int side = 0; side < 2; ++side) {               // side 0: cell i (face on its + side); 1: cell i+1
+                        const int ic = i + side;
+                        if (ic < 0 || ic > nd - 1) continue;
+                        size_t c = d == 0 ? o.idx(ic, ta, tb) : d == 1 ? o.idx(ta, ic, tb) : o.idx(ta, tb, ic);
+                        const double sgn = side == 0 ? -1.0 : 1.0;
+                        double W0[4], W1[4];
+                        for (int q = 0; q < 4; ++q) {
+                            W0[q] = UL[q * N + c];
+                            W1[q] = W0[q] + sgn * 6.0 * lam * CC[d][f * 5 + q];
+                        }
+                        const double g0 = g_adm(W0), g1 = g_adm(W1);
+                        const double delta = std::min(1e-8 * W0[0], g0);
+                        if (!(g1 >= delta)) {
+                            double t = (g0 - delta) / (g0 - g1);
+                            if (!(t >= 0.0)) t = 0.0;
+                            if (t < th) th = t;
+                        }
+                    }
+                    TH[d][f] = th;
+                    if (th < 1.0) ++nlim;
+                }
+    }
+    o.nlim += nlim;
+    for (int d = 0; d < 3; ++d) {
+        const int nd = d == 0 ? nx : d == 1 ? ny : nz, na = d == 0 ? ny : nx, nb = d == 2 ? ny : nz;
+#pragma omp parallel for collapse(2)
+        for (int tb = 0; tb < nb; ++tb)
+            for (int ta = 0; ta < na; ++ta)
+                for (int i = 0; i < nd; ++i) {
+                    size_t c = d == 0 ? o.idx(i, ta, tb) : d == 1 ? o.idx(ta, i, tb) : o.idx(ta, tb, i);
+                    const size_t f = ((size_t)tb * na + ta) * (nd + 1) + i;
+                    for (int q = 0; q < nf; ++q) {
+                        double fr = FL[d][(f + 1) * 5 + q] + TH[d][f + 1] * CC[d][(f + 1) * 5 + q];
+                        double fl = FL[d][f * 5 + q] + TH[d][f] * CC[d][f * 5 + q];
+                        L[q * N + c] -= (fr - fl) / o.dx;
+                    }
+                }
+    }
+}
 
 // L(U, t_s): O3, O4, O6, O7, O8.  `stage_c` = c_s in t_s = (n + c_s) dt.
 void eval_rhs(Oracle& o, const std::vector<double>& U, double stage_c, std::vector<double>& L, int stage_no,
@@ -322,6 +435,8 @@ void eval_rhs(Oracle& o, const std::vector<double>& U, double stage_c, std::vect
     o.has_nan |= has_nan;
 
     std::fill(L.begin(), L.end(), 0.0);
+    if (o.limiter) limited_divergence(o, U, L);
+    else
     // O6 + O7, direction by direction, all from the same U (R1: unsplit)
     for (int d = 0; d < 3; ++d) {
         const int nd = d == 0 ? nx : d == 1 ? ny : nz;
@@ -445,7 +560,7 @@ void* oracle_create(int nx, int ny, int nz, double dx, double dt, int nfields, d
     Oracle* o = new Oracle();
     o->nx = nx; o->ny = ny; o->nz = nz; o->nf = nfields; o->dx = dx; o->dt = dt;
     o->eps = weno_eps; o->delta = v_cap_delta; o->e_floor = e_floor;
-    o->step = 0; o->ncap = 0; o->has_nan = 0; o->order = 7; o->sigma = 0.0;
+    o->step = 0; o->ncap = 0; o->has_nan = 0; o->order = 7; o->sigma = 0.0; o->limiter = 0; o->nlim = 0;
     size_t T = o->N() * nfields;
     o->U.assign(T, 0.0); o->U1.assign(T, 0.0); o->U2.assign(T, 0.0); o->L.assign(T, 0.0);
     o->P.resize(o->N());
@@ -455,6 +570,13 @@ void* oracle_create(int nx, int ny, int nz, double dx, double dt, int nfields, d
     return o;
 }
 void oracle_destroy(void* h) { delete (Oracle*)h; }
+// positivity-preserving flux limiter on/off (R16, f-1); returns the cumulative count of limited faces so far
+long long oracle_set_limiter(void* h, int on) {
+    Oracle* o = (Oracle*)h;
+    o->limiter = on ? 1 : 0;
+    return o->nlim;
+}
+long long oracle_limited_faces(void* h) { return ((Oracle*)h)->nlim; }
 // width of the Gaussian deposit [fm] (R15, f-3); 0 restores the point deposit of R7
 int oracle_set_deposit_width(void* h, double sigma) {
     if (!(sigma >= 0.0)) return 1;
@@ -472,7 +594,7 @@ int oracle_set_weno_order(void* h, int order) {
 void oracle_set_state(void* h, const double* U) {
     Oracle* o = (Oracle*)h;
     std::copy(U, U + o->N() * o->nf, o->U.begin());
-    o->step = 0; o->ncap = 0; o->has_nan = 0;
+    o->step = 0; o->ncap = 0; o->has_nan = 0; o->nlim = 0;
     for (int d = 0; d < 4; ++d) o->deposited[d] = 0.0;
     for (size_t J = 0; J < o->jets.size(); ++J) o->jets[J].step_added = 0;
 }

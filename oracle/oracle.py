@@ -59,6 +59,10 @@ def lib():
         L.oracle_weno7_parts.argtypes = [dp, d, dp, dp, dp, dp]
         L.oracle_interface_flux.argtypes = [i, i, dp, d, d, d, d, dp]
         L.oracle_interface_flux_order.argtypes = [i, i, dp, d, d, d, d, i, dp]
+        L.oracle_set_limiter.restype = ll
+        L.oracle_set_limiter.argtypes = [p, i]
+        L.oracle_limited_faces.restype = ll
+        L.oracle_limited_faces.argtypes = [p]
         L.oracle_set_deposit_width.restype = i
         L.oracle_set_deposit_width.argtypes = [p, d]
         L.oracle_set_weno_order.restype = i
@@ -126,6 +130,13 @@ class Oracle:
     def clear_jets(self):
         self.L.oracle_clear_jets(self.h)
         self.njets = 0
+
+    def set_limiter(self, on=True):
+        """Positivity-preserving flux limiter (reading R16)."""
+        self.L.oracle_set_limiter(self.h, 1 if on else 0)
+
+    def limited_faces(self):
+        return self.L.oracle_limited_faces(self.h)
 
     def set_deposit_width(self, sigma):
         """Gaussian deposit of width sigma [fm] (reading R15); 0 = point deposit (R7)."""
