@@ -116,7 +116,7 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_slab_run(cfg, nzs, steps, warmup=0, order=7, sigma=0.0):
+def oracle_slab_run(cfg, nzs, steps, warmup=0, order=7, sigma=0.0, limiter=False):
     """Oracle on the central nzs planes of config `cfg`'s initial condition; returns (cells, seconds, threads)."""
     from oracle import oracle as O
     c = S.CONFIGS[cfg]
@@ -128,6 +128,7 @@ def oracle_slab_run(cfg, nzs, steps, warmup=0, order=7, sigma=0.0):
     for pos, d in c["jets"]:
         o.add_jet(pos, d, S.KAPPA_RAD, S.KAPPA_COLL, S.CR_OVER_CF)
     o.set_deposit_width(sigma)
+    o.set_limiter(limiter)
     if warmup:
         o.step(warmup)
     t0 = time.perf_counter()
@@ -144,10 +145,10 @@ def run_reference(args, rank):
     cfg = args.config
     c = S.CONFIGS[cfg]
     # size the slab so that (K + W) steps take about two minutes: calibrate on one step of 8 planes
-    cells8, t8, threads = oracle_slab_run(cfg, 8, 1, order=args.weno_order, sigma=args.deposit_sigma)
+    cells8, t8, threads = oracle_slab_run(cfg, 8, 1, order=args.weno_order, sigma=args.deposit_sigma, limiter=args.limiter)
     budget = 120.0
     nzs = int(min(c["n"][2], max(8, 8 * int(budget / (t8 * (args.steps + args.warmup)) + 1e-9))))
-    cells, secs, threads = oracle_slab_run(cfg, nzs, args.steps, args.warmup, order=args.weno_order, sigma=args.deposit_sigma)
+    cells, secs, threads = oracle_slab_run(cfg, nzs, args.steps, args.warmup, order=args.weno_order, sigma=args.deposit_sigma, limiter=args.limiter)
     value = cells * args.steps / secs
     sample = "%dx%dx%d central slab of config %d's IC + jet, %d RK3 steps" % (c["n"][0], c["n"][1], nzs, cfg,
                                                                               args.steps)
@@ -167,7 +168,7 @@ def workload_config(args, cfg):
     return {"workload": "BASELINE config %d: %dx%dx%d, dx=%g fm, dt=%g fm/c, nf=%d, p=e/3, ellipsoidal flow + %d jet(s), "
                         "outflow ghosts" % (cfg, c["n"][0], c["n"][1], c["n"][2], c["dx"], c["dt"], c["nf"],
                                             len(c["jets"])),
-            "cells": int(np.prod(c["n"])), "config_steps": c["steps"], "weno_order": getattr(args, "weno_order", 7), "deposit_sigma_fm": getattr(args, "deposit_sigma", 0.0),
+            "cells": int(np.prod(c["n"])), "config_steps": c["steps"], "weno_order": getattr(args, "weno_order", 7), "deposit_sigma_fm": getattr(args, "deposit_sigma", 0.0), "limiter": bool(getattr(args, "limiter", False)),
             "parallelism": "replicas x%d" % args.gpus,
             "l2": "state (%.0f MiB per copy) exceeds L2; no flush needed" %
                   (np.prod(c["n"]) * c["nf"] * (args.precision // 8) / 2 ** 20)}
@@ -183,6 +184,7 @@ def main():
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
     ap.add_argument("--weno-order", type=int, default=7, choices=[7, 5])
     ap.add_argument("--deposit-sigma", type=float, default=0.0, help="Gaussian deposit width [fm] (R15); 0 = one cell")
+    ap.add_argument("--limiter", action="store_true", help="positivity-preserving flux limiter (R16, f-1); fp64 only")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -227,6 +229,7 @@ def main():
         g.add_jet(pos, d, S.KAPPA_RAD, S.KAPPA_COLL, S.CR_OVER_CF)
 
     g.set_deposit_width(args.deposit_sigma)
+    g.set_limiter(args.limiter)
 
     # ---- measured ALU peak of this GPU, same run
     peak_tf = H.measure_alu_peak(args.precision, 200.0, stream.cuda_stream)
@@ -306,7 +309,7 @@ def main():
             "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.precision == 64 else "f32",
             "data": "synthetic", "config": workload_config(args, cfg), "clocks": clocks,
             "gpu_launches": int(launches), "roofline": roof,
-            "diag": {"ncap": dg["ncap"], "alpha": dg["alpha"].tolist(), "deposited_E_GeV": float(dg["deposited"][0])},
+            "diag": {"limited_faces": g.limited_faces(), "ncap": dg["ncap"], "alpha": dg["alpha"].tolist(), "deposited_E_GeV": float(dg["deposited"][0])},
         }
         if e2e:
             line["e2e"] = {"value": job_value(world, cells, args.steps, e2e_max), "unit": UNIT,
@@ -314,7 +317,7 @@ def main():
                            "what": "hydro_set_state(host) + hydro_step(K) + hydro_get_fields(host), pinned buffers; "
                                    "bytes are the one upload / one download spread over K steps"}
         if not args.no_cpu_baseline and world == 1:
-            cells_s, secs, threads = oracle_slab_run(cfg, 16, 2, order=args.weno_order, sigma=args.deposit_sigma)
+            cells_s, secs, threads = oracle_slab_run(cfg, 16, 2, order=args.weno_order, sigma=args.deposit_sigma, limiter=args.limiter)
             line["cpu_baseline"] = {"value": cells_s * 2 / secs, "unit": UNIT, "cores": threads, "kind": "oracle",
                                     "sample": "%dx%dx16 central slab of config %d's IC + jet, 2 RK3 steps (%.1f s)" %
                                               (c["n"][0], c["n"][1], cfg, secs)}

@@ -74,6 +74,15 @@ int hydro_set_state(hydro_t *h, const void *U, int memspace);
 int hydro_add_jet(hydro_t *h, double x0, double y0, double z0, double dirx, double diry, double dirz,
                   double kappa_rad, double kappa_coll, double cr_over_cf, int *id);
 int hydro_clear_jets(hydro_t *h);
+/* Positivity-preserving flux limiter on/off (default off; fp64 only, HYDRO_EINVAL in fp32).  Reading R16 (
+ * SURVEY 8(f) f-1; PAPER.md:25/:58 cite the positivity-preserving FD-WENO scheme without details): every interface flux is
+ * F^L + theta (F^H - F^L) with F^L the first-order Lax-Friedrichs flux and one theta in [0,1] per face, chosen from the
+ * concavity of g(U) = E - |M| around the first-order update so that E > |M| is kept (for 3 alpha dt/dx <= 1).  Costs one
+ * extra kernel per stage and ~2 blocks/SM instead of 3 in the sweeps.  hydro_get_limited_faces: cumulative number of
+ * (face, stage) events with theta < 1.  Synchronises. */
+int hydro_set_limiter(hydro_t *h, int enable);
+int hydro_get_limited_faces(hydro_t *h, long long *n);
+
 /* Width sigma >= 0 [fm] of the jets' deposit (all jets of the handle).  0 (default): the delta function of eq. (2) is one
  * cell (R7).  > 0: a normalised Gaussian of that width around the jet position, sampled on the (2R+1)^3 cells around
  * the R7 cell, R = ceil(3 sigma/dx) clamped to [1, 8] (reading R15). */

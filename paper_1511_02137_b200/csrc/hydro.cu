@@ -22,6 +22,7 @@ struct hydro {
     long long N, Np;                    // interior cells; field stride nxp*ny*nz
     double dx, dt, weno_eps, delta, e_floor;
     double sigma;                       // Gaussian deposit width [fm]; 0 = point deposit
+    int limiter;                        // 1: positivity-preserving flux limiter (R16; fp64 only)
     size_t esz;                         // bytes per real
     cudaStream_t stream;
     bool own_stream;
@@ -123,51 +124,67 @@ int buf_index(const hydro* h, const void* U) {
 
 // One ring sweep (hydro_sweep_ring.cuh).  `Us` must be one of the three state buffers; `out_map` is the tensor map
 // (for direction DIR) of the buffer the result is stored / reduced into; `un_map` that of U^n (OUT_COMBINE).
-template <typename R, int ORDER, int DIR, int OUT, int NF>
+// LIM = 1 (fp64 only): the limited scheme of R16, U^L is read from h->L.
+template <typename R, int ORDER, int LIM, int DIR, int OUT, int NF>
 int launch_ring_nf(hydro* h, const void* Us, int slot, const CUtensorMap* out_map, const CUtensorMap* un_map, double coef,
                    double rk_a, double rk_b) {
-    const int b = buf_index(h, Us);
-    if (b < 0) return HYDRO_ESTATE;
-    RingMaps m;
-    m.U = h->mapU[b][DIR]; m.W = h->mapW[DIR]; m.P = h->mapP[DIR]; m.Out = *out_map; m.Un = un_map ? *un_map : *out_map;
-    RingArgs a;
-    a.diag = h->diag; a.slot = slot; a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.seg_len = h->seg_len[DIR];
-    a.eps_eff = (ORDER == 5 ? 48.0 : 144.0) * h->weno_eps; a.coef = coef; a.dt = h->dt; a.rk_a = rk_a; a.rk_b = rk_b;
-    const int nlane = DIR == 0 ? h->ny : h->nx;
-    const int other = DIR == 2 ? h->ny : h->nz;
-    dim3 grid((unsigned)(((nlane + 31) / 32) * other), (unsigned)h->tma_nseg[DIR], 1);
-    dim3 block(32, NF, 1);
-    {
-        Timer t(h, HYDRO_K_SWEEP_X + DIR);
-        k_sweep_ring<R, ORDER, DIR, OUT, NF><<<grid, block, ring_smem_bytes(NF, OUT, sizeof(R)), h->stream>>>(m, a);
+    if constexpr (LIM && sizeof(R) != 8) return HYDRO_ESTATE;
+    else {
+        const int b = buf_index(h, Us);
+        if (b < 0) return HYDRO_ESTATE;
+        RingMaps m;
+        m.U = h->mapU[b][DIR]; m.W = h->mapW[DIR]; m.P = h->mapP[DIR]; m.Out = *out_map; m.Un = un_map ? *un_map : *out_map;
+        m.UL = h->mapL[DIR];
+        RingArgs a;
+        a.diag = h->diag; a.slot = slot; a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.seg_len = h->seg_len[DIR];
+        a.eps_eff = (ORDER == 5 ? 48.0 : 144.0) * h->weno_eps; a.coef = coef; a.dt = h->dt; a.rk_a = rk_a; a.rk_b = rk_b;
+        a.k3lam = 3.0 * h->dt / h->dx; a.nlim = &h->diag->nlim_total;
+        const int nlane = DIR == 0 ? h->ny : h->nx;
+        const int other = DIR == 2 ? h->ny : h->nz;
+        dim3 grid((unsigned)(((nlane + 31) / 32) * other), (unsigned)h->tma_nseg[DIR], 1);
+        dim3 block(32, NF, 1);
+        {
+            Timer t(h, HYDRO_K_SWEEP_X + DIR);
+            k_sweep_ring<R, ORDER, LIM, DIR, OUT, NF><<<grid, block, ring_smem_bytes(NF, OUT, sizeof(R), LIM), h->stream>>>(m, a);
+        }
+        h->launches += 1;
+        CK(cudaGetLastError());
+        return HYDRO_OK;
     }
-    h->launches += 1;
-    CK(cudaGetLastError());
-    return HYDRO_OK;
 }
 
+template <typename R, int LIM, int DIR, int OUT>
+int launch_ring_lim(hydro* h, const void* Us, int slot, const CUtensorMap* out_map, const CUtensorMap* un_map, double coef,
+                    double rk_a, double rk_b) {
+    if (h->order == 5)
+        return h->nf == 4 ? launch_ring_nf<R, 5, LIM, DIR, OUT, 4>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b)
+                          : launch_ring_nf<R, 5, LIM, DIR, OUT, 5>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b);
+    return h->nf == 4 ? launch_ring_nf<R, 7, LIM, DIR, OUT, 4>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b)
+                      : launch_ring_nf<R, 7, LIM, DIR, OUT, 5>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b);
+}
 template <typename R, int DIR, int OUT>
 int launch_ring(hydro* h, const void* Us, int slot, const CUtensorMap* out_map, const CUtensorMap* un_map, double coef,
                 double rk_a, double rk_b) {
-    if (h->order == 5)
-        return h->nf == 4 ? launch_ring_nf<R, 5, DIR, OUT, 4>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b)
-                          : launch_ring_nf<R, 5, DIR, OUT, 5>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b);
-    return h->nf == 4 ? launch_ring_nf<R, 7, DIR, OUT, 4>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b)
-                      : launch_ring_nf<R, 7, DIR, OUT, 5>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b);
+    return h->limiter ? launch_ring_lim<R, 1, DIR, OUT>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b)
+                      : launch_ring_lim<R, 0, DIR, OUT>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b);
 }
 
-template <typename R, int DIR, int OUT, int NF>
+template <typename R, int LIM, int DIR, int OUT, int NF>
 int set_smem_attr() {
-    return (cudaFuncSetAttribute(k_sweep_ring<R, 7, DIR, OUT, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 ring_smem_bytes(NF, OUT, sizeof(R))) == cudaSuccess ? 0 : 1) +
-           (cudaFuncSetAttribute(k_sweep_ring<R, 5, DIR, OUT, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 ring_smem_bytes(NF, OUT, sizeof(R))) == cudaSuccess ? 0 : 1);
+    if constexpr (LIM && sizeof(R) != 8) return 0;
+    else
+        return (cudaFuncSetAttribute(k_sweep_ring<R, 7, LIM, DIR, OUT, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     ring_smem_bytes(NF, OUT, sizeof(R), LIM)) == cudaSuccess ? 0 : 1) +
+               (cudaFuncSetAttribute(k_sweep_ring<R, 5, LIM, DIR, OUT, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     ring_smem_bytes(NF, OUT, sizeof(R), LIM)) == cudaSuccess ? 0 : 1);
 }
 template <typename R, int NF>
 int set_smem_attrs() {
-    return set_smem_attr<R, 0, OUT_STORE, NF>() + set_smem_attr<R, 0, OUT_COMBINE1, NF>() +
-           set_smem_attr<R, 0, OUT_COMBINE, NF>() + set_smem_attr<R, 1, OUT_REDUCE, NF>() +
-           set_smem_attr<R, 2, OUT_REDUCE, NF>();
+    return set_smem_attr<R, 0, 0, OUT_STORE, NF>() + set_smem_attr<R, 0, 0, OUT_COMBINE1, NF>() +
+           set_smem_attr<R, 0, 0, OUT_COMBINE, NF>() + set_smem_attr<R, 0, 1, OUT_REDUCE, NF>() +
+           set_smem_attr<R, 0, 2, OUT_REDUCE, NF>() + set_smem_attr<R, 1, 0, OUT_COMBINE1, NF>() +
+           set_smem_attr<R, 1, 0, OUT_COMBINE, NF>() + set_smem_attr<R, 1, 1, OUT_REDUCE, NF>() +
+           set_smem_attr<R, 1, 2, OUT_REDUCE, NF>();
 }
 
 // 4-D tensor map (x, y, z, field) of one SoA buffer with `nfb` fields; box given per dimension
@@ -274,6 +291,36 @@ int eval_stage_ring(hydro* h, const void* Uin, int slot, int stage, double stage
                     void* Uout, const void* Un, double rk_a, double rk_b) {
     const double hid = 0.5 / h->dx;
     int rc;
+    if (h->limiter) {
+        // R16: U^L (first-order update) into h->L, then the sweeps add only theta x (WENO correction) to it
+        LowArgs<R> la;
+        la.U = (const R*)Uin; la.P = (const R*)h->P; la.W = (const R*)h->W; la.UL = (R*)h->L; la.diag = h->diag; la.slot = slot;
+        la.nx = h->nx; la.ny = h->ny; la.nz = h->nz; la.nxp = h->nxp; la.nf = h->nf; la.N = h->N; la.Np = h->Np;
+        la.lam = (R)(h->dt / h->dx);
+        if (h->ny > 65535 || h->nz > 65535) return HYDRO_EINVAL;
+        {
+            Timer t(h, HYDRO_K_PRIM);
+            k_lowup<R><<<dim3((unsigned)((h->nx + 127) / 128), (unsigned)h->ny, (unsigned)h->nz), 128, 0, h->stream>>>(la);
+        }
+        h->launches += 1;
+        CK(cudaGetLastError());
+        if (!Uout) {
+            // hydro_eval_rhs: limited Euler update into a free state buffer, L = (update - U_s) / dt into another
+            void* Ue = h->buf[(h->cur + 1) % 3];
+            void* Ld = h->buf[(h->cur + 2) % 3];
+            const int be = buf_index(h, Ue);
+            if ((rc = launch_ring<R, 0, OUT_COMBINE1>(h, Uin, slot, &h->mapU[be][0], 0, hid, 0.0, 1.0)) != HYDRO_OK) return rc;
+            if ((rc = launch_source<R>(h, slot, stage, stage_c, commit, rk_weight, Ue, h->dt)) != HYDRO_OK) return rc;
+            if ((rc = launch_ring<R, 1, OUT_REDUCE>(h, Uin, slot, &h->mapU[be][1], 0, h->dt * hid, 0.0, 0.0)) != HYDRO_OK) return rc;
+            if ((rc = launch_ring<R, 2, OUT_REDUCE>(h, Uin, slot, &h->mapU[be][2], 0, h->dt * hid, 0.0, 0.0)) != HYDRO_OK) return rc;
+            const long long n = h->Np * h->nf;
+            long long bl = (n + 255) / 256;
+            if (bl > (long long)h->num_sms * 16) bl = (long long)h->num_sms * 16;
+            k_diff<R><<<(unsigned)bl, 256, 0, h->stream>>>((const R*)Ue, (const R*)Uin, (R*)Ld, n, (R)(1.0 / h->dt));
+            CK(cudaGetLastError());
+            return HYDRO_OK;
+        }
+    }
     if (Uout) {
         const int bo = buf_index(h, Uout), bn = Un ? buf_index(h, Un) : -1;
         if (bo < 0 || (Un && bn < 0)) return HYDRO_ESTATE;
@@ -382,6 +429,7 @@ int hydro_create(hydro_t** out, int nx, int ny, int nz, double dx, double dt, co
     h->N = (long long)nx * ny * nz;
     h->order = o.weno_order == 5 ? 5 : 7;
     h->sigma = 0.0;
+    h->limiter = 0;
     h->dx = dx; h->dt = dt;
     h->weno_eps = o.weno_eps > 0 ? o.weno_eps : 1e-6;
     h->delta = o.v_cap_delta > 0 ? o.v_cap_delta : (o.precision == 64 ? 1e-10 : 1e-5);
@@ -477,6 +525,22 @@ int hydro_add_jet(hydro_t* h, double x0, double y0, double z0, double dirx, doub
     return HYDRO_OK;
 }
 
+int hydro_set_limiter(hydro_t* h, int enable) {
+    if (!h) return HYDRO_EINVAL;
+    if (enable && h->prec != 64) return HYDRO_EINVAL;                  // delta = 1e-8 E is below fp32 resolution
+    h->limiter = enable ? 1 : 0;
+    return HYDRO_OK;
+}
+
+int hydro_get_limited_faces(hydro_t* h, long long* n) {
+    if (!h || !n) return HYDRO_EINVAL;
+    Diag d;
+    CK(cudaMemcpyAsync(&d, h->diag, sizeof(Diag), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    *n = (long long)d.nlim_total;
+    return HYDRO_OK;
+}
+
 int hydro_set_deposit_width(hydro_t* h, double sigma) {
     if (!h || !(sigma >= 0.0) || !std::isfinite(sigma)) return HYDRO_EINVAL;
     h->sigma = sigma;
@@ -521,7 +585,7 @@ int hydro_eval_rhs(hydro_t* h, double stage_c, void* out, int memspace) {
     if (!h || !out || (memspace != HYDRO_MEM_HOST && memspace != HYDRO_MEM_DEVICE)) return HYDRO_EINVAL;
     int rc = h->prec == 64 ? eval_rhs_impl<double>(h, stage_c) : eval_rhs_impl<float>(h, stage_c);
     if (rc != HYDRO_OK) return rc;
-    return copy_out(h, h->L, out, memspace);
+    return copy_out(h, h->limiter ? h->buf[(h->cur + 2) % 3] : h->L, out, memspace);
 }
 
 int hydro_get_diag(hydro_t* h, double alpha[3], double* cfl, long long* ncap, int* has_nan, double deposited[4],

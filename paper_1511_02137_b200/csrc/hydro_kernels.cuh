@@ -28,6 +28,7 @@ struct Diag {
     DiagSlot slot[2];
     unsigned long long ncap_total;
     unsigned long long nan_total;
+    unsigned long long nlim_total;      // limiter (R16): faces with theta < 1, all stages
     double alpha_last[3];               // alpha of the last evaluated stage
     double deposited[4];                // jets: total (E, Mx, My, Mz) deposited [GeV]
     double last_q[3][MAX_JETS];         // q^s of every jet in the stages of the last step
@@ -248,6 +249,60 @@ __global__ void __launch_bounds__(256) k_prims_out(const R* __restrict__ U, R* _
             out[4 * Np + c] = U[4 * Np + c] * Real<R>::sqrt_(om);
         }
     }
+}
+
+// ------------------------------------------------------------------------------------------------ limiter: U^L (R16, f-1)
+// First-order Lax-Friedrichs update  U^L = U - (dt/dx) sum_d (F^L_{i+1/2} - F^L_{i-1/2}),
+// F^L_{i+1/2} = [(F_i + alpha U_i) + (F_{i+1} - alpha U_{i+1})] / 2, neighbours clamped (zero-gradient ghosts).
+// One thread per cell, all fields; the 6 neighbours come through L1/L2.  Launch: grid (ceil(nx/128), ny, nz) x 128.
+template <typename R>
+struct LowArgs {
+    const R* U; const R* P; const R* W; R* UL;
+    const Diag* diag;
+    int slot, nx, ny, nz, nxp, nf;
+    long long N, Np;
+    R lam;                       // dt / dx
+};
+
+template <typename R>
+__global__ void __launch_bounds__(128) k_lowup(LowArgs<R> a) {
+    typedef Real<R> T;
+    R alpha[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) alpha[d] = T::from_bits(a.diag->slot[a.slot].alpha_bits[d]);
+    // grid = (x tiles, ny, nz): no integer division per cell
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+    if (i < a.nx) {
+        const long long c = ((long long)k * a.ny + j) * a.nxp + i;
+        R acc[5], Uc[5];
+        for (int q = 0; q < a.nf; ++q) { Uc[q] = a.U[q * a.Np + c]; acc[q] = R(0); }
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const int id = d == 0 ? i : d == 1 ? j : k, nd = d == 0 ? a.nx : d == 1 ? a.ny : a.nz;
+            const long long st = d == 0 ? 1 : d == 1 ? a.nxp : (long long)a.nxp * a.ny;
+            const long long cm = id > 0 ? c - st : c, cp = id < nd - 1 ? c + st : c;
+            // sum over the two faces: (F^L_+ - F^L_-) = [ (F_p - alpha U_p) - (F_m + alpha U_m) ] / 2 + alpha U_c
+            const R vdp = a.U[(1 + d) * a.Np + cp] * a.W[cp], vdm = a.U[(1 + d) * a.Np + cm] * a.W[cm];
+            for (int q = 0; q < a.nf; ++q) {
+                const R up = a.U[q * a.Np + cp], um = a.U[q * a.Np + cm];
+                R Fp, Fm;
+                if (q == 0) { Fp = a.U[(1 + d) * a.Np + cp]; Fm = a.U[(1 + d) * a.Np + cm]; }
+                else {
+                    Fp = up * vdp; Fm = um * vdm;
+                    if (q == 1 + d) { Fp += a.P[cp]; Fm += a.P[cm]; }
+                }
+                acc[q] += R(0.5) * ((Fp - alpha[d] * up) - (Fm + alpha[d] * um)) + alpha[d] * Uc[q];
+            }
+        }
+        for (int q = 0; q < a.nf; ++q) a.UL[q * a.Np + c] = T::fma_(-a.lam, acc[q], Uc[q]);
+    }
+}
+
+// out = (A - B) / dt over the interior cells: L of the limited scheme for hydro_eval_rhs, from the limited Euler update
+template <typename R>
+__global__ void __launch_bounds__(256) k_diff(const R* __restrict__ A, const R* __restrict__ B, R* __restrict__ out, long long n, R inv_dt) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < n; c += stride) out[c] = (A[c] - B[c]) * inv_dt;
 }
 
 // ------------------------------------------------------------------------------------------------ a-5: jet source

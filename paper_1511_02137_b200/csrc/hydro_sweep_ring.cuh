@@ -87,9 +87,10 @@ __device__ __forceinline__ void tma_wait_all0() { asm volatile("cp.async.bulk.wa
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // shared-memory plan of one launch (host and device agree through these functions); units: reals
-__host__ __device__ constexpr int ring_stage_reals(int nf) { return (nf + 2) * RING_SUB; }
-__host__ __device__ constexpr int ring_smem_bytes(int nf, int out, int esz) {
-    return (RING_NSTAGE * ring_stage_reals(nf)            // input ring
+__host__ __device__ constexpr int ring_stage_reals(int nf, int lim = 0) { return (nf + 2 + (lim ? nf : 0)) * RING_SUB; }
+__host__ __device__ constexpr int ring_smem_bytes(int nf, int out, int esz, int lim = 0) {
+    return (RING_NSTAGE * ring_stage_reals(nf, lim)       // input ring (+ U^L tiles with the limiter)
+            + (lim ? (nf + 1) * RING_SUB : 0)              // limiter: flux-correction tiles of all fields + theta tile
             + 2 * nf * RING_SUB                            // two output tiles
             + (out == OUT_COMBINE ? 2 * nf * RING_SUB : 0) // two U^n tiles
             + RING_SUB) * esz                              // one tile of zeros
@@ -102,7 +103,8 @@ __host__ __device__ constexpr int ring_smem_bytes(int nf, int out, int esz) {
 #define RING_F32_BLOCKS 6
 #endif
 // resident blocks per SM the kernels are compiled for (registers: 65536 / (32 NF threads x blocks))
-__host__ __device__ constexpr int ring_blocks_per_sm(int nf, int esz, int out = OUT_COMBINE) {
+__host__ __device__ constexpr int ring_blocks_per_sm(int nf, int esz, int out = OUT_COMBINE, int lim = 0) {
+    if (lim) return nf == 4 ? 2 : 1;                       // 88-104 KB (nf = 4), 106-126 KB (nf = 5) of shared memory
     // nf = 5 in fp64: 3 blocks (<= 136 registers, 64 KB) except the combine kernel with its U^n tiles (84 KB): 2
     return esz == 8 ? (nf == 4 ? RING_F64_BLOCKS : (out != OUT_COMBINE ? 3 : 2)) : (nf == 4 ? RING_F32_BLOCKS : 4);
 }
@@ -111,6 +113,7 @@ struct RingMaps {
     CUtensorMap U, W, P;       // loads: stage state (NF fields per box), W and P (one field per box)
     CUtensorMap Un;            // load : U^n at the output cells (OUT_COMBINE)
     CUtensorMap Out;           // store / reduce target (NF fields per box)
+    CUtensorMap UL;            // load : first-order update U^L (limiter, R16)
 };
 
 struct RingArgs {
@@ -121,6 +124,8 @@ struct RingArgs {
     double eps_eff;            // WENO7: 144 * weno_eps (the split fluxes are carried as 2 f^+-, beta as 36 beta); WENO5: 48 * weno_eps
     double coef;               // OUT_STORE / OUT_REDUCE: c = [b dt] / (2 dx);  OUT_COMBINE*: 1 / (2 dx)
     double dt, rk_a, rk_b;
+    double k3lam;              // limiter: 3 dt/dx (6 dt/dx times the correction C = corr/2 carried as 2 F_hat)
+    unsigned long long* nlim;  // limiter: count of faces with theta < 1
 };
 
 // element offset inside a sub-tile of march row r (0..7) for this lane
@@ -256,8 +261,10 @@ __device__ __forceinline__ void weno5_diff(R D0, R D1, R D2, R D3, R E0, R E1, R
 //   plus  side: cells i-3..i+3 = slots r-7..r-1, centre i   = V[r-4]
 //   minus side: cells i-2..i+4 = slots r-6..r,   centre i+1 = V[r-3], stencil order reversed (D_j = -d[5-j], ...)
 //   ORDER 5: plus cells i-2..i+2 = slots r-6..r-2 (centre V[r-4]); minus cells i-1..i+3 = slots r-5..r-1 reversed
+// rot_flux_parts: 2 F_hat = vsum + corr with vsum = 2 f+_i + 2 f-_{i+1} (twice the first-order Lax-Friedrichs flux) and
+// corr the high-order WENO correction (the limiter of R16 scales corr by theta).
 template <int r, int ORDER, typename R>
-__device__ __forceinline__ R rot_flux(const RotWin<R>& wp, const RotWin<R>& wm, R eps) {
+__device__ __forceinline__ void rot_flux_parts(const RotWin<R>& wp, const RotWin<R>& wm, R eps, R& vsum, R& corr) {
 #define SL(k) (((r) + (k) + 16) & 7)
     R bp, np_, dp, bm, nm, dm;
     if (ORDER == 5) {
@@ -278,8 +285,15 @@ __device__ __forceinline__ R rot_flux(const RotWin<R>& wp, const RotWin<R>& wm, 
     R x;
     if (sizeof(R) == 8) x = (R)(fma((double)np_, (double)dm, (double)nm * (double)dp) * rcp_cubic((double)dp * (double)dm));
     else x = (R)fmaf((float)np_, rcp_ulp((float)dp), (float)nm * rcp_ulp((float)dm));
-    return Real<R>::fma_((bp + bm) + x, ORDER == 5 ? R(1.0 / 6.0) : R(1.0 / 12.0), wp.V[SL(-4)] + wm.V[SL(-3)]);
+    corr = ((bp + bm) + x) * (ORDER == 5 ? R(1.0 / 6.0) : R(1.0 / 12.0));
+    vsum = wp.V[SL(-4)] + wm.V[SL(-3)];
 #undef SL
+}
+template <int r, int ORDER, typename R>
+__device__ __forceinline__ R rot_flux(const RotWin<R>& wp, const RotWin<R>& wm, R eps) {
+    R vsum, corr;
+    rot_flux_parts<r, ORDER, R>(wp, wm, eps, vsum, corr);
+    return vsum + corr;
 }
 
 // per-thread view of one input stage: element pointers with the lane offset folded in
@@ -301,10 +315,67 @@ struct RowPtr {
     }
 };
 
-template <typename R, int ORDER, int DIR, int OUT, int NF>
+// ------------------------------------------------------------------------------------------------ limiter (R16, f-1)
+// theta of one cell for the face state W1 = W0 + sgn * a (W0 = U^L of the cell, a = 6 dt/dx C of the face):
+// 1 if g(W1) >= delta, else (g(W0) - delta) / (g(W0) - g(W1)), g = E - |M|, delta = min(1e-8 E0, g(W0)).
+// The common case is decided on squares (no square root).
+template <typename R>
+__device__ __forceinline__ R theta_cell(const R W0[4], const R a[4], R sgn) {
+    const R E0 = W0[0], M02 = W0[1] * W0[1] + W0[2] * W0[2] + W0[3] * W0[3];
+    const R d8 = R(1e-8) * E0;
+    const R W1[4] = {Real<R>::fma_(sgn, a[0], W0[0]), Real<R>::fma_(sgn, a[1], W0[1]), Real<R>::fma_(sgn, a[2], W0[2]),
+                     Real<R>::fma_(sgn, a[3], W0[3])};
+    const R M12 = W1[1] * W1[1] + W1[2] * W1[2] + W1[3] * W1[3];
+    const R t0 = E0 - d8, t1 = W1[0] - d8;
+    if (t0 >= R(0) && t0 * t0 >= M02 && t1 >= R(0) && t1 * t1 >= M12) return R(1);
+    const R g0 = E0 - Real<R>::sqrt_(M02), g1 = W1[0] - Real<R>::sqrt_(M12);
+    const R delta = d8 < g0 ? d8 : g0;
+    if (g1 >= delta) return R(1);
+    R t = (g0 - delta) / (g0 - g1);
+    if (!(t >= R(0))) t = R(0);
+    return t < R(1) ? t : R(1);
+}
+
+// theta of the face of chunk row r (between march cells i = cm + r - 4 and i + 1) for this lane: reads the corrections of
+// the four energy-momentum fields from the exchange tiles and U^L of the two cells from the ring (rows r-4, r-3; the
+// previous chunk's stage for negative rows).  Cells outside the grid impose no condition.  Returns 1 if theta < 1.
+template <int r, int DIR, int NF, typename R>
+__device__ __forceinline__ int theta_row(const R* st, const R* stp, const R* xc_all, R* th, int lane, int cm, int nd, R k3lam) {
+    constexpr int ULB = NF + 2;
+    const int o = sub_off<DIR, R>(r, lane);
+    R a[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) a[q] = k3lam * xc_all[q * RING_SUB + o];
+    const int i = cm + r - 4;
+    R theta = R(1);
+    if (i >= 0 && i <= nd - 1) {
+        constexpr int rl = (r + 4) & 7;
+        const R* s = r < 4 ? stp : st;
+        const int ol = sub_off<DIR, R>(rl, lane);
+        const R W0[4] = {s[(ULB + 0) * RING_SUB + ol], s[(ULB + 1) * RING_SUB + ol], s[(ULB + 2) * RING_SUB + ol],
+                         s[(ULB + 3) * RING_SUB + ol]};
+        const R t = theta_cell<R>(W0, a, R(-1));
+        theta = t < theta ? t : theta;
+    }
+    if (i + 1 >= 0 && i + 1 <= nd - 1) {
+        constexpr int rr = (r + 5) & 7;
+        const R* s = r < 3 ? stp : st;
+        const int orr = sub_off<DIR, R>(rr, lane);
+        const R W0[4] = {s[(ULB + 0) * RING_SUB + orr], s[(ULB + 1) * RING_SUB + orr], s[(ULB + 2) * RING_SUB + orr],
+                         s[(ULB + 3) * RING_SUB + orr]};
+        const R t = theta_cell<R>(W0, a, R(1));
+        theta = t < theta ? t : theta;
+    }
+    th[o] = theta;
+    return theta < R(1) ? 1 : 0;
+}
+
+template <typename R, int ORDER, int LIM, int DIR, int OUT, int NF>
 struct SweepCtx {
     RotWin<R> wp, wm;
     R fhat_prev;
+    R* xc_own;                             // limiter: this field's flux-correction tile
+    const R* th;                           // limiter: theta tile
     R alpha, c3, eps, coef, dt, rk_a, rk_b, kE;
     // current chunk
     RowPtr<DIR, R> pu, pmd, pa, pw, pp;    // own field, normal momentum, A operand, W (or zeros), P (or zeros)
@@ -327,10 +398,27 @@ struct SweepCtx {
         rot_push<r, ORDER, R>(wp, T::fma_(alpha, u, F), c3, eps);
         rot_push<r, ORDER, R>(wm, T::fma_(-alpha, u, F), c3, eps);
     }
+    // limiter, phase A: the row's high-order correction goes to the exchange tile
+    template <int r>
+    __device__ __forceinline__ void corr_store() {
+        load_push<r>();
+        R vsum, corr;
+        rot_flux_parts<r, ORDER, R>(wp, wm, eps, vsum, corr);
+        xc_own[sub_off<DIR, R>(r, lane)] = corr;
+    }
+    // limiter, phase C: the first-order part of every flux is already inside U^L; what is left is theta * corr
+    template <int r>
+    __device__ __forceinline__ void emit_lim() {
+        const int o = sub_off<DIR, R>(r, lane);
+        emit_with<r>(th[o] * xc_own[o]);
+    }
     template <int r>
     __device__ __forceinline__ void emit() {
+        emit_with<r>(rot_flux<r, ORDER, R>(wp, wm, eps));
+    }
+    template <int r>
+    __device__ __forceinline__ void emit_with(const R fhat) {
         typedef Real<R> T;
-        const R fhat = rot_flux<r, ORDER, R>(wp, wm, eps);
         const R mdiv = (fhat_prev - fhat) * coef;
         fhat_prev = fhat;
         R o;
@@ -350,19 +438,21 @@ struct SweepCtx {
     }
 };
 
-template <typename R, int ORDER, int DIR, int OUT, int NF>
-__global__ void __launch_bounds__(32 * NF, ring_blocks_per_sm(NF, sizeof(R), OUT))
+template <typename R, int ORDER, int LIM, int DIR, int OUT, int NF>
+__global__ void __launch_bounds__(32 * NF, ring_blocks_per_sm(NF, sizeof(R), OUT, LIM))
 k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
     // 1024-byte alignment: the swizzle pattern is a function of the absolute shared address
     extern __shared__ __align__(1024) unsigned char smem[];
-    constexpr int STAGE_REALS = ring_stage_reals(NF);
+    constexpr int STAGE_REALS = ring_stage_reals(NF, LIM);
     constexpr uint32_t STAGE_BYTES = STAGE_REALS * sizeof(R);
     constexpr uint32_t UN_BYTES = NF * RING_SUB * sizeof(R);
     R* stages = (R*)smem;
     R* outt = stages + RING_NSTAGE * STAGE_REALS;                      // two output tiles of NF sub-tiles
     R* unt = outt + 2 * NF * RING_SUB;                                 // OUT_COMBINE: two U^n tiles
     R* zeros = unt + (OUT == OUT_COMBINE ? 2 * NF * RING_SUB : 0);
-    uint64_t* full = (uint64_t*)(zeros + RING_SUB);
+    R* xc = zeros + RING_SUB;                                          // limiter: NF correction tiles, then the theta tile
+    R* tht = xc + (LIM ? NF * RING_SUB : 0);
+    uint64_t* full = (uint64_t*)(tht + (LIM ? RING_SUB : 0));
 
     const int lane = threadIdx.x, f = threadIdx.y;
     const bool leader = (lane == 0 && f == 0);
@@ -405,6 +495,7 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
         tma_load_4d(dst, &maps.U, &full[st], c0, c1, c2, 0);
         tma_load_4d(dst + NF * RING_SUB, &maps.W, &full[st], c0, c1, c2, 0);
         tma_load_4d(dst + (NF + 1) * RING_SUB, &maps.P, &full[st], c0, c1, c2, 0);
+        if (LIM) tma_load_4d(dst + (NF + 2) * RING_SUB, &maps.UL, &full[st], c0, c1, c2, 0);
         if (with_un) {
             coords(s0 + (m - 1) * RING_CH, c0, c1, c2);                // the cells chunk m emits
             tma_load_4d(unt + (m & 1) * NF * RING_SUB, &maps.Un, &full[st], c0, c1, c2, 0);
@@ -423,7 +514,10 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
         if (nchunks > 1) issue(1);
     }
 
-    SweepCtx<R, ORDER, DIR, OUT, NF> cx;
+    SweepCtx<R, ORDER, LIM, DIR, OUT, NF> cx;
+    cx.xc_own = xc + f * RING_SUB;
+    cx.th = tht;
+    int nlim_local = 0;
     cx.wp.clear();
     cx.wm.clear();
     cx.fhat_prev = R(0);
@@ -476,9 +570,9 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
         cx.pa.set(is_energy ? st + (1 + DIR) * RING_SUB : st + f * RING_SUB, lane);
         cx.pw.set(is_energy ? zeros : st + NF * RING_SUB, lane);
         cx.pp.set(is_normal ? st + (NF + 1) * RING_SUB : zeros, lane);
-        if (OUT == OUT_COMBINE1 || OUT == OUT_COMBINE) {
-            cx.pus[0].set(stp + f * RING_SUB, lane);
-            cx.pus[1].set(st + f * RING_SUB, lane);
+        if (OUT == OUT_COMBINE1 || OUT == OUT_COMBINE) {           // the state the stage's own part is added to: U_s, or U^L
+            cx.pus[0].set(stp + (LIM ? NF + 2 + f : f) * RING_SUB, lane);
+            cx.pus[1].set(st + (LIM ? NF + 2 + f : f) * RING_SUB, lane);
         }
         if (OUT == OUT_COMBINE) cx.pun.set(unt + (m & 1) * NF * RING_SUB + f * RING_SUB, lane);
         cx.out = outt + (m & 1) * NF * RING_SUB + f * RING_SUB;
@@ -487,10 +581,42 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
             // warm-up chunk: cells s0-4 .. s0+3 fill both windows; the last row gives the interface s0 - 1/2
             cx.template load_push<0>(); cx.template load_push<1>(); cx.template load_push<2>(); cx.template load_push<3>();
             cx.template load_push<4>(); cx.template load_push<5>(); cx.template load_push<6>(); cx.template load_push<7>();
-            cx.fhat_prev = rot_flux<7, ORDER, R>(cx.wp, cx.wm, cx.eps);
-        } else {
+            if (!LIM) cx.fhat_prev = rot_flux<7, ORDER, R>(cx.wp, cx.wm, cx.eps);
+            else {
+                R vsum, corr;
+                rot_flux_parts<7, ORDER, R>(cx.wp, cx.wm, cx.eps, vsum, corr);
+                cx.xc_own[sub_off<DIR, R>(7, lane)] = corr;
+                __syncthreads();
+                if (f == 0) {
+                    const int n1 = theta_row<7, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, (R)a.k3lam);
+                    if (s0 == 0) nlim_local += n1;                     // inner segment starts are counted by the segment before
+                }
+                __syncthreads();
+                cx.fhat_prev = tht[sub_off<DIR, R>(7, lane)] * corr;
+            }
+        } else if (!LIM) {
             cx.template row<0>(); cx.template row<1>(); cx.template row<2>(); cx.template row<3>();
             cx.template row<4>(); cx.template row<5>(); cx.template row<6>(); cx.template row<7>();
+        } else {
+            // R16: (A) corrections of all fields to shared memory, (B) one theta per face from all fields, (C) emit
+            cx.template corr_store<0>(); cx.template corr_store<1>(); cx.template corr_store<2>(); cx.template corr_store<3>();
+            cx.template corr_store<4>(); cx.template corr_store<5>(); cx.template corr_store<6>(); cx.template corr_store<7>();
+            __syncthreads();
+            const R k3 = (R)a.k3lam;
+            switch (f) {
+                case 0: nlim_local += theta_row<0, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, k3) +
+                                      theta_row<1, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, k3); break;
+                case 1: nlim_local += theta_row<2, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, k3) +
+                                      theta_row<3, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, k3); break;
+                case 2: nlim_local += theta_row<4, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, k3) +
+                                      theta_row<5, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, k3); break;
+                case 3: nlim_local += theta_row<6, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, k3) +
+                                      theta_row<7, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, k3); break;
+                default: break;
+            }
+            __syncthreads();
+            cx.template emit_lim<0>(); cx.template emit_lim<1>(); cx.template emit_lim<2>(); cx.template emit_lim<3>();
+            cx.template emit_lim<4>(); cx.template emit_lim<5>(); cx.template emit_lim<6>(); cx.template emit_lim<7>();
         }
     }
     fence_proxy_async();
@@ -499,6 +625,10 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
     if (leader) {
         if (nchunks > 1) flush(nchunks - 1);
         tma_wait_all0();
+    }
+    if (LIM) {
+        for (int off = 16; off > 0; off >>= 1) nlim_local += __shfl_xor_sync(0xffffffffu, nlim_local, off);
+        if (lane == 0 && nlim_local) atomicAdd(a.nlim, (unsigned long long)nlim_local);
     }
 }
 

@@ -22,7 +22,7 @@ FIELDS_CONSERVED, FIELDS_PRIMITIVE = 0, 1
 K_NAMES = ("prim", "sweep_x", "sweep_y", "sweep_z", "source")
 
 # every symbol include/hydro.h declares (tests check that the library exports all of them)
-SYMBOLS = ("hydro_create", "hydro_destroy", "hydro_set_state", "hydro_add_jet", "hydro_clear_jets", "hydro_set_deposit_width", "hydro_step",
+SYMBOLS = ("hydro_create", "hydro_destroy", "hydro_set_state", "hydro_add_jet", "hydro_clear_jets", "hydro_set_deposit_width", "hydro_set_limiter", "hydro_get_limited_faces", "hydro_step",
            "hydro_synchronize", "hydro_get_fields", "hydro_eval_rhs", "hydro_get_diag", "hydro_get_last_stage_q",
            "hydro_set_profiling", "hydro_get_kernel_times", "hydro_launch_count", "hydro_sweep_path", "hydro_measure_alu_peak",
            "hydro_strerror", "hydro_last_cuda_error")
@@ -63,6 +63,10 @@ def load():
     L.hydro_add_jet.argtypes = [vp] + [d] * 9 + [C.POINTER(i)]
     L.hydro_clear_jets.restype = i
     L.hydro_clear_jets.argtypes = [vp]
+    L.hydro_set_limiter.restype = i
+    L.hydro_set_limiter.argtypes = [vp, i]
+    L.hydro_get_limited_faces.restype = i
+    L.hydro_get_limited_faces.argtypes = [vp, C.POINTER(ll)]
     L.hydro_set_deposit_width.restype = i
     L.hydro_set_deposit_width.argtypes = [vp, d]
     L.hydro_step.restype = i
@@ -182,6 +186,14 @@ class Hydro:
     def clear_jets(self):
         self._ck(self.L.hydro_clear_jets(self.h), "hydro_clear_jets")
         self.njets = 0
+
+    def set_limiter(self, on=True):
+        self._ck(self.L.hydro_set_limiter(self.h, 1 if on else 0), "hydro_set_limiter")
+
+    def limited_faces(self):
+        n = C.c_longlong()
+        self._ck(self.L.hydro_get_limited_faces(self.h, C.byref(n)), "hydro_get_limited_faces")
+        return n.value
 
     def set_deposit_width(self, sigma):
         self._ck(self.L.hydro_set_deposit_width(self.h, float(sigma)), "hydro_set_deposit_width")

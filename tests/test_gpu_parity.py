@@ -449,6 +449,83 @@ def test_smeared_deposit_run(H, oracle, prec, tol):
     g.close(), o.close()
 
 
+# ------------------------------------------------------------------------------------------------ flux limiter (f-1)
+def _rough_state(n, seed, vmax=0.98):
+    rng = np.random.default_rng(seed)
+    shape = (n[2], n[1], n[0])
+    e = 10.0 ** rng.uniform(-2, 2, shape)
+    vm = rng.uniform(0, vmax, shape)
+    d = rng.normal(size=(3,) + shape)
+    d /= np.linalg.norm(d, axis=0)
+    u = vm / np.sqrt(1 - vm * vm) * d
+    return S.prim_to_cons(e, u[0], u[1], u[2])
+
+
+@pytest.mark.parametrize("n", [(32, 32, 32), (37, 19, 23), (9, 5, 3), (72, 12, 40)])
+@pytest.mark.parametrize("order", [7, 5])
+def test_limiter_rhs_parity(H, oracle, n, order):
+    """R16 on rough admissible data (the limiter acts on a large share of the faces) and on smooth data with a jet:
+    L of the limited scheme, GPU vs oracle."""
+    for kind in ("rough", "smooth"):
+        if kind == "rough":
+            U0 = _rough_state(n, 5)
+            jets = []
+        else:
+            c = S.scaled_config(0, n)
+            U0 = S.make_state(c)
+            jets = [((-0.12, 0.03, 0.0), (1.0, 0.5, -0.25))]
+        g = H.Hydro(*n, 0.1, 0.02, weno_order=order)
+        o = oracle.Oracle(*n, 0.1, 0.02, weno_order=order)
+        g.set_state(U0), o.set_state(U0)
+        g.set_limiter(True), o.set_limiter(True)
+        for pos, d in jets:
+            g.add_jet(pos, d), o.add_jet(pos, d)
+        Lg, Lo = g.eval_rhs(0.5), o.eval_rhs(0.5)
+        scale = np.max(np.abs(Lo), axis=(1, 2, 3))
+        for f in range(4):
+            # L is recovered from the limited Euler update: (U' - U)/dt costs ulp(U)/dt of absolute accuracy
+            tol = 1e-11 * max(scale[f], scale[0]) + 4e-16 * np.max(np.abs(U0[f])) / 0.02
+            assert np.max(np.abs(Lg[f] - Lo[f])) <= tol, (kind, f)
+        ng, no = g.limited_faces(), o.limited_faces()
+        if kind == "rough":
+            assert no > 0 and abs(ng - no) <= max(2, 0.01 * no)
+        else:
+            assert ng == no == 0
+        g.close(), o.close()
+
+
+def test_limiter_runs(H, oracle):
+    """The jet/cap case with the limiter: parity after the run, the cap never fires, the state stays admissible;
+    rough data: admissible on the GPU as in the oracle."""
+    c = S.scaled_config(2, (64, 32, 32))
+    c["jets"] = [((-2.0, 0.0, 0.0), (1.0, 0.0, 0.0))]
+    steps = 40
+    c, U0, g, o = make_pair(H, oracle, c)
+    g.set_limiter(True), o.set_limiter(True)
+    g.step(steps), o.step(steps)
+    Ug, Uo = g.get_fields(), o.get_fields()
+    errs = r13(Ug, Uo)
+    assert max(errs) < 1e-8, errs                     # theta = (g0 - delta)/(g0 - g1) amplifies rounding where it acts
+    dg, do = compare_diag(g, o, steps)
+    assert dg["ncap"] == do["ncap"] == 0
+    assert (Ug[0] - np.sqrt(Ug[1] ** 2 + Ug[2] ** 2 + Ug[3] ** 2)).min() > 0
+    ng, no = g.limited_faces(), o.limited_faces()
+    assert no > 0 and abs(ng - no) <= max(3, 0.02 * no)
+    g.close(), o.close()
+    n = (24, 20, 16)
+    U0 = _rough_state(n, 11)
+    g, o = H.Hydro(*n, 0.1, 0.02), oracle.Oracle(*n, 0.1, 0.02)
+    g.set_state(U0), o.set_state(U0)
+    g.set_limiter(True), o.set_limiter(True)
+    g.step(4), o.step(4)
+    Ug, Uo = g.get_fields(), o.get_fields()
+    assert (Ug[0] - np.sqrt(Ug[1] ** 2 + Ug[2] ** 2 + Ug[3] ** 2)).min() > 0 and g.diag()["ncap"] == 0
+    assert max(r13(Ug, Uo)) < 1e-7
+    g.close(), o.close()
+    with pytest.raises(H.HydroError):
+        H.Hydro(8, 8, 8, 0.1, 0.02, precision=32).set_limiter(True)
+
+
 # ------------------------------------------------------------------------------------------------ invariants on the GPU
 def test_gpu_uniform_state_and_symmetry(H):
     n = (40, 24, 17)
