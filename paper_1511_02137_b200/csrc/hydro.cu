@@ -23,6 +23,7 @@ struct hydro {
     double dx, dt, weno_eps, delta, e_floor;
     double sigma;                       // Gaussian deposit width [fm]; 0 = point deposit
     int limiter;                        // 1: positivity-preserving flux limiter (R16; fp64 only)
+    int nz_global, k_offset, own_lo, own_hi;   // z-slab decomposition (f-4); defaults: nz, 0, 0, nz
     size_t esz;                         // bytes per real
     cudaStream_t stream;
     bool own_stream;
@@ -104,6 +105,7 @@ int launch_prim(hydro* h, const void* U, int slot) {
     CK(cudaMemsetAsync(&h->diag->slot[slot], 0, sizeof(DiagSlot), h->stream));
     PrimArgs<R> a;
     a.U = (const R*)U; a.P = (R*)h->P; a.W = (R*)h->W; a.diag = h->diag; a.slot = slot; a.N = h->N; a.Np = h->Np; a.nx = h->nx; a.nxp = h->nxp;
+    a.own_lo = (long long)h->own_lo * h->nx * h->ny; a.own_hi = (long long)h->own_hi * h->nx * h->ny;
     a.e_floor = (R)h->e_floor; a.one_minus_delta = (R)(1.0 - h->delta);
     long long blocks = (h->N + 255) / 256;
     long long cap = (long long)h->num_sms * 8;
@@ -274,6 +276,7 @@ int launch_source(hydro* h, int slot, int stage, double stage_c, bool commit, do
     SourceArgs s;
     s.diag = h->diag; s.jets = h->jets_dev; s.njets = (int)h->jets.size(); s.slot = slot; s.stage = stage;
     s.commit = commit ? 1 : 0; s.nx = h->nx; s.ny = h->ny; s.nz = h->nz; s.nxp = h->nxp; s.N = h->Np; s.step = h->step;
+    s.nz_global = h->nz_global; s.k_offset = h->k_offset; s.own_lo = h->own_lo; s.own_hi = h->own_hi;
     s.stage_c = stage_c; s.dx = h->dx; s.dt = h->dt; s.rk_weight = rk_weight; s.scale = scale; s.sigma = h->sigma;
     {
         Timer t(h, HYDRO_K_SOURCE);
@@ -378,6 +381,33 @@ int step_impl(hydro* h, int nsteps) {
     return HYDRO_OK;
 }
 
+// ---- stage-level stepping (z-slab decomposition, f-4): the caller exchanges alpha / halos between the calls
+struct StagePlan { void* in; void* out; const void* un; int slot; double c, w, a, b; };
+StagePlan stage_plan(hydro* h, int s) {
+    void* Un = h->buf[h->cur];
+    void* Ua = h->buf[(h->cur + 1) % 3];
+    void* Ub = h->buf[(h->cur + 2) % 3];
+    const int slot = h->prim_slot;
+    StagePlan p;
+    if (s == 0) { p.in = Un; p.out = Ua; p.un = 0; p.slot = slot; p.c = 0.0; p.w = 1.0 / 6.0; p.a = 0.0; p.b = 1.0; }
+    else if (s == 1) { p.in = Ua; p.out = Ub; p.un = Un; p.slot = slot ^ 1; p.c = 1.0; p.w = 1.0 / 6.0; p.a = 0.75; p.b = 0.25; }
+    else { p.in = Ub; p.out = Un; p.un = Un; p.slot = slot; p.c = 0.5; p.w = 2.0 / 3.0; p.a = 1.0 / 3.0; p.b = 2.0 / 3.0; }
+    return p;
+}
+template <typename R>
+int stage_prims_impl(hydro* h, int s) {
+    const StagePlan p = stage_plan(h, s);
+    return launch_prim<R>(h, p.in, p.slot);
+}
+template <typename R>
+int stage_sweeps_impl(hydro* h, int s) {
+    const StagePlan p = stage_plan(h, s);
+    int rc = eval_stage<R>(h, p.in, p.slot, s, p.c, true, p.w, p.out, p.un, p.a, p.b);
+    if (rc != HYDRO_OK) return rc;
+    if (s == 2) { h->step += 1; h->prim_slot ^= 1; h->prims_valid = false; }
+    return HYDRO_OK;
+}
+
 template <typename R>
 int eval_rhs_impl(hydro* h, double stage_c) {
     int rc;
@@ -430,6 +460,7 @@ int hydro_create(hydro_t** out, int nx, int ny, int nz, double dx, double dt, co
     h->order = o.weno_order == 5 ? 5 : 7;
     h->sigma = 0.0;
     h->limiter = 0;
+    h->nz_global = nz; h->k_offset = 0; h->own_lo = 0; h->own_hi = nz;
     h->dx = dx; h->dt = dt;
     h->weno_eps = o.weno_eps > 0 ? o.weno_eps : 1e-6;
     h->delta = o.v_cap_delta > 0 ? o.v_cap_delta : (o.precision == 64 ? 1e-10 : 1e-5);
@@ -522,6 +553,66 @@ int hydro_add_jet(hydro_t* h, double x0, double y0, double z0, double dirx, doub
     h->jets.push_back(j);
     h->jets_dirty = true;
     if (id) *id = (int)h->jets.size() - 1;
+    return HYDRO_OK;
+}
+
+int hydro_set_slab(hydro_t* h, int nz_global, int k_offset, int own_lo, int own_hi) {
+    if (!h || nz_global < h->nz || k_offset < 0 || k_offset + h->nz > nz_global || own_lo < 0 || own_hi > h->nz || own_lo >= own_hi)
+        return HYDRO_EINVAL;
+    // an interior slab end must carry the 4 halo planes the stencil needs
+    if ((k_offset > 0 && own_lo < 4) || (k_offset + h->nz < nz_global && h->nz - own_hi < 4)) return HYDRO_EINVAL;
+    h->nz_global = nz_global; h->k_offset = k_offset; h->own_lo = own_lo; h->own_hi = own_hi;
+    h->prims_valid = false;
+    return HYDRO_OK;
+}
+
+int hydro_stage_prims(hydro_t* h, int s) {
+    if (!h || s < 0 || s > 2) return HYDRO_EINVAL;
+    return h->prec == 64 ? stage_prims_impl<double>(h, s) : stage_prims_impl<float>(h, s);
+}
+
+int hydro_stage_sweeps(hydro_t* h, int s) {
+    if (!h || s < 0 || s > 2) return HYDRO_EINVAL;
+    return h->prec == 64 ? stage_sweeps_impl<double>(h, s) : stage_sweeps_impl<float>(h, s);
+}
+
+int hydro_stage_alpha(hydro_t* h, int s, int set, double alpha[3]) {
+    if (!h || s < 0 || s > 2 || !alpha) return HYDRO_EINVAL;
+    const StagePlan p = stage_plan(h, s);
+    unsigned long long bits[3];
+    if (set) {
+        for (int d = 0; d < 3; ++d) {
+            if (!(alpha[d] >= 0.0)) return HYDRO_EINVAL;
+            if (h->prec == 64) { double x = alpha[d]; memcpy(&bits[d], &x, 8); }
+            else { float x = (float)alpha[d]; unsigned int u; memcpy(&u, &x, 4); bits[d] = u; }
+        }
+        CK(cudaMemcpyAsync(h->diag->slot[p.slot].alpha_bits, bits, sizeof bits, cudaMemcpyHostToDevice, h->stream));
+        CK(cudaStreamSynchronize(h->stream));
+        return HYDRO_OK;
+    }
+    CK(cudaMemcpyAsync(bits, h->diag->slot[p.slot].alpha_bits, sizeof bits, cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    for (int d = 0; d < 3; ++d) {
+        if (h->prec == 64) { double x; memcpy(&x, &bits[d], 8); alpha[d] = x; }
+        else { unsigned int u = (unsigned int)bits[d]; float x; memcpy(&x, &u, 4); alpha[d] = x; }
+    }
+    return HYDRO_OK;
+}
+
+int hydro_halo(hydro_t* h, int s, int side, int unpack, void* dev_buf) {
+    if (!h || s < 0 || s > 2 || (side != 0 && side != 1) || !dev_buf) return HYDRO_EINVAL;
+    const StagePlan p = stage_plan(h, s == 2 ? 2 : s);
+    // stage s's OUTPUT state; after stage 2 the plan has rotated (prim_slot flipped) but buf[cur] is still U^{n+1}
+    char* base = (char*)(s == 0 ? h->buf[(h->cur + 1) % 3] : s == 1 ? h->buf[(h->cur + 2) % 3] : h->buf[h->cur]);
+    (void)p;
+    const size_t plane = (size_t)h->nxp * h->ny * h->esz, width = 4 * plane, fpitch = (size_t)h->Np * h->esz;
+    int k0;                                   // first of the 4 planes
+    if (!unpack) k0 = side == 0 ? h->own_lo : h->own_hi - 4;            // owned boundary planes -> buffer
+    else k0 = side == 0 ? h->own_lo - 4 : h->own_hi;                    // buffer -> halo planes
+    if (k0 < 0 || k0 + 4 > h->nz || h->own_hi - h->own_lo < 4) return HYDRO_EINVAL;
+    char* planes = base + (size_t)k0 * plane;
+    if (!unpack) CK(cudaMemcpy2DAsync(dev_buf, width, planes, fpitch, width, (size_t)h->nf, cudaMemcpyDeviceToDevice, h->stream));
+    else CK(cudaMemcpy2DAsync(planes, fpitch, dev_buf, width, width, (size_t)h->nf, cudaMemcpyDeviceToDevice, h->stream));
     return HYDRO_OK;
 }
 

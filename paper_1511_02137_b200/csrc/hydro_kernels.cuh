@@ -138,6 +138,7 @@ struct PrimArgs {
     int slot;
     int nx, nxp;       // cells per row, row pitch
     long long N, Np;   // interior cells, field stride
+    long long own_lo, own_hi;   // cap events are counted for interior cells in [own_lo, own_hi) only (slab halos excluded)
     R e_floor, one_minus_delta;
 };
 
@@ -157,13 +158,13 @@ __global__ void __launch_bounds__(256) k_prim(PrimArgs<R> a) {
     const R* __restrict__ U1 = a.U + a.Np;
     const R* __restrict__ U2 = a.U + 2 * a.Np;
     const R* __restrict__ U3 = a.U + 3 * a.Np;
-    auto cell = [&](long long c, R E, R Mx, R My, R Mz) {
+    auto cell = [&](long long c, long long c0, R E, R Mx, R My, R Mz) {
         R p, wt;
         int lim;
         con2prim<R>(E, Mx, My, Mz, a.e_floor, a.one_minus_delta, p, wt, lim);
         a.P[c] = p;
         a.W[c] = wt;
-        ncap += lim;
+        ncap += (c0 >= a.own_lo && c0 < a.own_hi) ? lim : 0;
         // finite check: x - x is 0 for finite x, NaN otherwise
         R chk = (E - E) + (Mx - Mx) + (My - My) + (Mz - Mz);
         bad |= (chk == R(0)) ? 0u : 1u;
@@ -186,12 +187,12 @@ __global__ void __launch_bounds__(256) k_prim(PrimArgs<R> a) {
         const long long p1 = pad_index(c, a.nx, a.nxp), p2 = pad_index(c + stride, a.nx, a.nxp);
         const R E = U0[p1], Mx = U1[p1], My = U2[p1], Mz = U3[p1];
         const R E2 = U0[p2], Mx2 = U1[p2], My2 = U2[p2], Mz2 = U3[p2];
-        cell(p1, E, Mx, My, Mz);
-        cell(p2, E2, Mx2, My2, Mz2);
+        cell(p1, c, E, Mx, My, Mz);
+        cell(p2, c + stride, E2, Mx2, My2, Mz2);
     }
     if (c < a.N) {
         const long long p1 = pad_index(c, a.nx, a.nxp);
-        cell(p1, U0[p1], U1[p1], U2[p1], U3[p1]);
+        cell(p1, c, U0[p1], U1[p1], U2[p1], U3[p1]);
     }
     // warp reduction by shuffles, then one atomic per warp on the bit pattern (non-negative reals order like
     // unsigned integers; the max is exact, hence order independent)
@@ -315,6 +316,7 @@ struct SourceArgs {
     const JetDev* jets;
     int njets, slot, stage, commit;    // commit: add the slot's cap/NaN counts to the totals, log q, accumulate deposits
     int nx, ny, nz, nxp;
+    int nz_global, k_offset, own_lo, own_hi;   // z-slab (f-4): global planes, global index of local plane 0, owned local planes
     long long N /* field stride Np */, step;
     double stage_c, dx, dt, rk_weight;
     double scale;                      // the deposit is added to `target` times this (1 for L, b dt for a stage state)
@@ -362,7 +364,9 @@ __global__ void __launch_bounds__(SOURCE_THREADS) k_source(SourceArgs a, const R
                          zj = __dadd_rn(jt.z0, __dmul_rn(jt.nz, ell));
             const int ci = jet_axis_index(xj, a.nx, a.dx);
             const int cj = jet_axis_index(yj, a.ny, a.dx);
-            const int ck = jet_axis_index(zj, a.nz, a.dx);
+            int ck = jet_axis_index(zj, a.nz_global, a.dx);
+            if (ck >= 0) { ck -= a.k_offset; if (ck >= a.nz) ck = -1; }        // global -> local plane; outside the local array: no deposit here
+            const bool owned = ck >= a.own_lo && ck < a.own_hi;
             double q = 0.0;
             if (ci >= 0 && cj >= 0 && ck >= 0) {
                 const long long c = ((long long)ck * a.ny + cj) * a.nxp + ci;
@@ -379,8 +383,8 @@ __global__ void __launch_bounds__(SOURCE_THREADS) k_source(SourceArgs a, const R
                 }
             }
             if (a.commit) {
-                if (J < MAX_JETS) dg->last_q[a.stage][J] = q;
-                const double amt = a.dt * a.rk_weight * q;
+                if (J < MAX_JETS) dg->last_q[a.stage][J] = owned ? q : 0.0;
+                const double amt = owned ? a.dt * a.rk_weight * q : 0.0;
                 dg->deposited[0] += amt;
                 dg->deposited[1] += amt * jt.nx;
                 dg->deposited[2] += amt * jt.ny;
@@ -399,14 +403,14 @@ __global__ void __launch_bounds__(SOURCE_THREADS) k_source(SourceArgs a, const R
             const int side = 2 * Rr + 1, ncell = side * side * side;
             const double inv2s2 = 1.0 / (2.0 * a.sigma * a.sigma);
             const double x0c = ((ci + 0.5) - 0.5 * a.nx) * a.dx - sh_pos[0], y0c = ((cj + 0.5) - 0.5 * a.ny) * a.dx - sh_pos[1],
-                         z0c = ((ck + 0.5) - 0.5 * a.nz) * a.dx - sh_pos[2];
+                         z0c = ((ck + a.k_offset + 0.5) - 0.5 * a.nz_global) * a.dx - sh_pos[2];
             const double r02 = x0c * x0c + y0c * y0c + z0c * z0c;
             auto weight = [&](int s, int& i2, int& j2, int& k2) {
                 const int di = s % side - Rr, dj = (s / side) % side - Rr, dk = s / (side * side) - Rr;
                 i2 = ci + di; j2 = cj + dj; k2 = ck + dk;
                 const double ddx = ((i2 + 0.5) - 0.5 * a.nx) * a.dx - sh_pos[0];
                 const double ddy = ((j2 + 0.5) - 0.5 * a.ny) * a.dx - sh_pos[1];
-                const double ddz = ((k2 + 0.5) - 0.5 * a.nz) * a.dx - sh_pos[2];
+                const double ddz = ((k2 + a.k_offset + 0.5) - 0.5 * a.nz_global) * a.dx - sh_pos[2];
                 return exp(-((ddx * ddx + ddy * ddy + ddz * ddz) - r02) * inv2s2);
             };
             double part = 0.0;
