@@ -46,7 +46,7 @@ FLOPS_STAGE_W5 = {4: 1820.0, 5: 2261.0}
 FLOPS_SWEEPS_STAGE_W5 = {4: 3 * (560.0 + 12.0) + 20.0, 5: 3 * (700.0 + 15.0) + 25.0}
 FP64_NOMINAL_TF = 148 * 64 * 2 * 1.965e9 / 1e12          # 148 SMs x 64 DFMA/clk x 2 x 1.965 GHz = 37.2
 # dram__bytes_read.sum + dram__bytes_write.sum per sweep launch at 256^3 fp64 nf=4, mean of the x (COMBINE), y and z
-# (REDUCE) kernels, from the one `ncu --set full` capture summarised in profiles/r1_c_ring_ncu_summary.txt
+# (REDUCE) kernels, from the one `ncu --set full` capture summarised in profiles/r1_g_ring_ncu_summary.txt
 NCU_TRAFFIC_SWEEP_256_F64_NF4 = (1.310e9 + 1.837e9 + 1.839e9) / 3.0
 
 
@@ -174,6 +174,54 @@ def workload_config(args, cfg):
                   (np.prod(c["n"]) * c["nf"] * (args.precision // 8) / 2 ** 20)}
 
 
+def run_decomposed(args, rank, world, local, barrier):
+    """--decompose: ONE grid of config `args.config` split into `world` z-slabs (paper_1511_02137_b200/slab.py); every
+    rank advances its slab, exchanging the Lax-Friedrichs speeds and 4 halo planes per face once per stage.  Strong
+    scaling: value = cells x steps / max-over-ranks time.  Device-timed on the handle's stream (everything between the
+    two events is host-synchronised per stage)."""
+    import torch
+    import torch.distributed as dist
+    from paper_1511_02137_b200 import hydro as H, slab as SL
+    cfg = args.config
+    c = S.CONFIGS[cfg]
+    cells = int(np.prod(c["n"]))
+    U0 = S.make_state(cfg).astype(np.float64 if args.precision == 64 else np.float32)
+    stream = torch.cuda.Stream()
+    sl = SL.Slab(H, c["n"], c["dx"], c["dt"], rank, world, nfields=c["nf"], precision=args.precision, stream=stream,
+                 weno_order=args.weno_order)
+    for pos, d in c["jets"]:
+        sl.g.add_jet(pos, d, S.KAPPA_RAD, S.KAPPA_COLL, S.CR_OVER_CF)
+    sl.g.set_deposit_width(args.deposit_sigma)
+    sl.g.set_limiter(args.limiter)
+    d_ = dist if world > 1 else None
+    sl.set_state(U0)
+    SL.run_distributed(sl, args.warmup, d_)
+    sl.set_state(U0)
+    sl.g.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0 = sl.g.launch_count()
+    barrier()
+    e0.record(stream)
+    SL.run_distributed(sl, args.steps, d_)
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    ms_max = max_over_ranks([ms], world, "cuda")[0]
+    dg = sl.g.diag()
+    if dg["has_nan"]:
+        raise SystemExit("bench.py: non-finite state after the timed run")
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": cells * args.steps / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f64" if args.precision == 64 else "f32",
+            "data": "synthetic", "config": dict(workload_config(args, cfg), parallelism="z-slabs x%d" % world),
+            "gpu_launches": int(sl.g.launch_count() - n0),
+            "halo_bytes_per_stage_per_face": int(sl.g.halo_reals() * (args.precision // 8)),
+        }), flush=True)
+    sl.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -184,6 +232,9 @@ def main():
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
     ap.add_argument("--weno-order", type=int, default=7, choices=[7, 5])
     ap.add_argument("--deposit-sigma", type=float, default=0.0, help="Gaussian deposit width [fm] (R15); 0 = one cell")
+    ap.add_argument("--decompose", action="store_true",
+                    help="with --gpus N > 1: split ONE grid into N z-slabs (strong scaling, halo exchange + MAX all-reduce "
+                         "over NCCL; DESIGN.md 9) instead of N independent replicas")
     ap.add_argument("--limiter", action="store_true", help="positivity-preserving flux limiter (R16, f-1); fp64 only")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -211,6 +262,12 @@ def main():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
+
+    if args.decompose:
+        run_decomposed(args, rank, world, local, barrier)
+        if world > 1:
+            dist.destroy_process_group()
+        return
 
     cfg = args.config
     c = S.CONFIGS[cfg]
@@ -301,7 +358,7 @@ def main():
                 "kernel_ms_per_step": {k: v["ms"] / args.steps for k, v in kt.items()},
                 "whole_path_frac": (fl_stage * 3 * value) / (peak_tf * 1e12),
                 "traffic": NCU_TRAFFIC_SWEEP_256_F64_NF4 if (cfg == 3 and args.precision == 64 and args.weno_order == 7) else None,
-                "traffic_source": "profiles/r1_c_ring_ncu_summary.txt (ncu --set full, dram read+write per launch)",
+                "traffic_source": "profiles/r1_g_ring_ncu_summary.txt (ncu --set full, dram read+write per launch)",
                 "algorithmic_bytes_per_launch": (nf + 2 + nf + nf * 2.0 / 9.0 + 2.0 / 3.0 * nf) * 8.0 * cells}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

@@ -74,6 +74,28 @@ int hydro_set_state(hydro_t *h, const void *U, int memspace);
 int hydro_add_jet(hydro_t *h, double x0, double y0, double z0, double dirx, double diry, double dirz,
                   double kappa_rad, double kappa_coll, double cr_over_cf, int *id);
 int hydro_clear_jets(hydro_t *h);
+/* ---- z-slab decomposition over several GPUs: one handle per rank -------------------------------
+ * The handle's grid is the rank's LOCAL array: its owned planes plus 4 halo planes towards each neighbouring rank (none
+ * at a physical boundary, where the zero-gradient ghosts of a-7 act).  hydro_set_slab: nz_global = planes of the whole
+ * grid, k_offset = global index of local plane 0, [own_lo, own_hi) = owned local planes (>= 4 of them; an interior end
+ * needs its 4 halo planes: HYDRO_EINVAL otherwise).  Jet positions stay global; cap events and jet bookkeeping are
+ * counted for owned planes only, so sums over ranks are the global figures.
+ * One RK3 step = for s in 0, 1, 2:
+ *     hydro_stage_prims(h, s)                      con2prim + LOCAL wavespeed maxima of stage s's input state
+ *     hydro_stage_alpha(h, s, 0, a); a = MAX over ranks; hydro_stage_alpha(h, s, 1, a)      (host round trip, 24 bytes)
+ *     hydro_stage_sweeps(h, s)                     sweeps + source + stage combination -> stage s's output state
+ *     hydro_halo(h, s, side, 0, buf)  pack the 4 owned boundary planes (side 0: low z, 1: high z) of that output state,
+ *                                     all fields, into the DEVICE buffer buf (nfields * 4 * ny * pitch reals, see
+ *                                     hydro_halo_reals); exchange with the neighbour; hydro_halo(h, s, side, 1, buf) unpacks
+ *                                     the neighbour's planes into the halo.  Asynchronous on the handle's stream.
+ * hydro_stage_sweeps(h, 2) advances the step counter.  Owned planes come out bitwise identical to the one-GPU run. */
+int hydro_set_slab(hydro_t *h, int nz_global, int k_offset, int own_lo, int own_hi);
+int hydro_stage_prims(hydro_t *h, int s);
+int hydro_stage_alpha(hydro_t *h, int s, int set, double alpha[3]);
+int hydro_stage_sweeps(hydro_t *h, int s);
+int hydro_halo(hydro_t *h, int s, int side, int unpack, void *dev_buf);
+long long hydro_halo_reals(const hydro_t *h);
+
 /* Positivity-preserving flux limiter on/off (default off; fp64 only, HYDRO_EINVAL in fp32).  Reading R16 (
  * SURVEY 8(f) f-1; PAPER.md:25/:58 cite the positivity-preserving FD-WENO scheme without details): every interface flux is
  * F^L + theta (F^H - F^L) with F^L the first-order Lax-Friedrichs flux and one theta in [0,1] per face, chosen from the

@@ -16,6 +16,7 @@
 
 using namespace hydro_dev;
 
+struct EvSpan { int cls; cudaEvent_t a, b; bool owns_a; };   // one profiled launch: [a, b] on the handle's stream
 struct hydro {
     int nx, ny, nz, nf, prec, order;    // order: 7 (WENO7, the paper's scheme) or 5 (its WENO5 variant)
     int nxp;                            // row pitch in reals: nx rounded up so that a row is a multiple of 16 bytes (TMA)
@@ -47,8 +48,9 @@ struct hydro {
     long long launches;
     // profiling
     bool profiling;
-    std::vector<std::pair<int, std::pair<cudaEvent_t, cudaEvent_t> > > ev_inflight;
-    std::vector<std::pair<cudaEvent_t, cudaEvent_t> > ev_pool;
+    std::vector<EvSpan> ev_inflight;
+    std::vector<cudaEvent_t> ev_pool;
+    cudaEvent_t chain_prev;             // end event of the previous profiled launch (0: start a new chain)
     double k_ms[HYDRO_K_COUNT];
     long long k_n[HYDRO_K_COUNT];
     std::string cuda_err;
@@ -70,34 +72,48 @@ int cuda_fail(hydro* h, cudaError_t e, const char* where) {
         if (e_ != cudaSuccess) return cuda_fail(h, e_, #call);          \
     } while (0)
 
-struct Timer {                          // brackets one launch with events when profiling is on
+// Per-launch device times when profiling is on: ONE event after every launch; a launch's start is the previous
+// launch's end event (launches of a step are back to back on the stream), so profiling costs one event per launch.
+cudaEvent_t get_event(hydro* h) {
+    cudaEvent_t e = 0;
+    if (!h->ev_pool.empty()) { e = h->ev_pool.back(); h->ev_pool.pop_back(); }
+    else cudaEventCreate(&e);
+    return e;
+}
+struct Timer {
     hydro* h;
-    int cls;
-    cudaEvent_t a, b;
+    EvSpan sp;
     bool on;
-    Timer(hydro* h_, int cls_) : h(h_), cls(cls_), a(0), b(0), on(h_->profiling) {
+    Timer(hydro* h_, int cls_) : h(h_), on(h_->profiling) {
         if (!on) return;
-        if (!h->ev_pool.empty()) { a = h->ev_pool.back().first; b = h->ev_pool.back().second; h->ev_pool.pop_back(); }
-        else { cudaEventCreate(&a); cudaEventCreate(&b); }
-        cudaEventRecord(a, h->stream);
+        sp.cls = cls_;
+        if (h->chain_prev) { sp.a = h->chain_prev; sp.owns_a = false; }
+        else { sp.a = get_event(h); sp.owns_a = true; cudaEventRecord(sp.a, h->stream); }
     }
     ~Timer() {
         if (!on) return;
-        cudaEventRecord(b, h->stream);
-        h->ev_inflight.push_back(std::make_pair(cls, std::make_pair(a, b)));
+        sp.b = get_event(h);
+        cudaEventRecord(sp.b, h->stream);
+        h->ev_inflight.push_back(sp);
+        h->chain_prev = sp.b;
     }
 };
 
 void drain_events(hydro* h) {
     for (size_t n = 0; n < h->ev_inflight.size(); ++n) {
+        const EvSpan& sp = h->ev_inflight[n];
         float ms = 0.f;
-        cudaEventSynchronize(h->ev_inflight[n].second.second);
-        cudaEventElapsedTime(&ms, h->ev_inflight[n].second.first, h->ev_inflight[n].second.second);
-        h->k_ms[h->ev_inflight[n].first] += ms;
-        h->k_n[h->ev_inflight[n].first] += 1;
-        h->ev_pool.push_back(h->ev_inflight[n].second);
+        cudaEventSynchronize(sp.b);
+        cudaEventElapsedTime(&ms, sp.a, sp.b);
+        h->k_ms[sp.cls] += ms;
+        h->k_n[sp.cls] += 1;
+    }
+    for (size_t n = 0; n < h->ev_inflight.size(); ++n) {
+        if (h->ev_inflight[n].owns_a) h->ev_pool.push_back(h->ev_inflight[n].a);
+        h->ev_pool.push_back(h->ev_inflight[n].b);
     }
     h->ev_inflight.clear();
+    h->chain_prev = 0;
 }
 
 template <typename R>
@@ -476,6 +492,7 @@ int hydro_create(hydro_t** out, int nx, int ny, int nz, double dx, double dt, co
     h->cur = 0; h->L = h->P = h->W = h->scratch = 0; h->diag = 0; h->jets_dev = 0;
     h->jets_dirty = false; h->step = 0; h->prim_slot = 0; h->prims_valid = false; h->launches = 0;
     h->profiling = false;
+    h->chain_prev = 0;
     for (int k = 0; k < HYDRO_K_COUNT; ++k) { h->k_ms[k] = 0; h->k_n[k] = 0; }
     int rc = HYDRO_OK;
     do {
@@ -518,7 +535,7 @@ void hydro_destroy(hydro_t* h) {
     if (!h) return;
     if (h->stream || !h->own_stream) cudaStreamSynchronize(h->stream);
     drain_events(h);
-    for (size_t n = 0; n < h->ev_pool.size(); ++n) { cudaEventDestroy(h->ev_pool[n].first); cudaEventDestroy(h->ev_pool[n].second); }
+    for (size_t n = 0; n < h->ev_pool.size(); ++n) cudaEventDestroy(h->ev_pool[n]);
     for (int b = 0; b < 3; ++b) cudaFree(h->buf[b]);
     cudaFree(h->L); cudaFree(h->P); cudaFree(h->W); cudaFree(h->scratch); cudaFree(h->diag); cudaFree(h->jets_dev);
     if (h->own_stream && h->stream) cudaStreamDestroy(h->stream);
@@ -616,6 +633,8 @@ int hydro_halo(hydro_t* h, int s, int side, int unpack, void* dev_buf) {
     return HYDRO_OK;
 }
 
+long long hydro_halo_reals(const hydro_t* h) { return h ? (long long)h->nf * 4 * h->ny * h->nxp : -1; }
+
 int hydro_set_limiter(hydro_t* h, int enable) {
     if (!h) return HYDRO_EINVAL;
     if (enable && h->prec != 64) return HYDRO_EINVAL;                  // delta = 1e-8 E is below fp32 resolution
@@ -647,6 +666,7 @@ int hydro_clear_jets(hydro_t* h) {
 
 int hydro_step(hydro_t* h, int nsteps) {
     if (!h || nsteps < 0) return HYDRO_EINVAL;
+    h->chain_prev = 0;                                              // other work may sit on the stream since the last launch
     return h->prec == 64 ? step_impl<double>(h, nsteps) : step_impl<float>(h, nsteps);
 }
 

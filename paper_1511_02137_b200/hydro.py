@@ -22,7 +22,8 @@ FIELDS_CONSERVED, FIELDS_PRIMITIVE = 0, 1
 K_NAMES = ("prim", "sweep_x", "sweep_y", "sweep_z", "source")
 
 # every symbol include/hydro.h declares (tests check that the library exports all of them)
-SYMBOLS = ("hydro_create", "hydro_destroy", "hydro_set_state", "hydro_add_jet", "hydro_clear_jets", "hydro_set_deposit_width", "hydro_set_limiter", "hydro_get_limited_faces", "hydro_step",
+SYMBOLS = ("hydro_create", "hydro_destroy", "hydro_set_state", "hydro_add_jet", "hydro_clear_jets", "hydro_set_deposit_width", "hydro_set_limiter", "hydro_get_limited_faces", "hydro_set_slab", "hydro_stage_prims",
+           "hydro_stage_alpha", "hydro_stage_sweeps", "hydro_halo", "hydro_halo_reals", "hydro_step",
            "hydro_synchronize", "hydro_get_fields", "hydro_eval_rhs", "hydro_get_diag", "hydro_get_last_stage_q",
            "hydro_set_profiling", "hydro_get_kernel_times", "hydro_launch_count", "hydro_sweep_path", "hydro_measure_alu_peak",
            "hydro_strerror", "hydro_last_cuda_error")
@@ -63,6 +64,18 @@ def load():
     L.hydro_add_jet.argtypes = [vp] + [d] * 9 + [C.POINTER(i)]
     L.hydro_clear_jets.restype = i
     L.hydro_clear_jets.argtypes = [vp]
+    L.hydro_set_slab.restype = i
+    L.hydro_set_slab.argtypes = [vp, i, i, i, i]
+    L.hydro_stage_prims.restype = i
+    L.hydro_stage_prims.argtypes = [vp, i]
+    L.hydro_stage_alpha.restype = i
+    L.hydro_stage_alpha.argtypes = [vp, i, i, dp]
+    L.hydro_stage_sweeps.restype = i
+    L.hydro_stage_sweeps.argtypes = [vp, i]
+    L.hydro_halo.restype = i
+    L.hydro_halo.argtypes = [vp, i, i, i, vp]
+    L.hydro_halo_reals.restype = ll
+    L.hydro_halo_reals.argtypes = [vp]
     L.hydro_set_limiter.restype = i
     L.hydro_set_limiter.argtypes = [vp, i]
     L.hydro_get_limited_faces.restype = i
@@ -186,6 +199,29 @@ class Hydro:
     def clear_jets(self):
         self._ck(self.L.hydro_clear_jets(self.h), "hydro_clear_jets")
         self.njets = 0
+
+    # -- z-slab decomposition (f-4): see include/hydro.h and paper_1511_02137_b200/slab.py
+    def set_slab(self, nz_global, k_offset, own_lo, own_hi):
+        self._ck(self.L.hydro_set_slab(self.h, nz_global, k_offset, own_lo, own_hi), "hydro_set_slab")
+
+    def stage_prims(self, s):
+        self._ck(self.L.hydro_stage_prims(self.h, s), "hydro_stage_prims")
+
+    def stage_alpha(self, s, alpha=None):
+        a = (C.c_double * 3)(*(alpha if alpha is not None else (0.0, 0.0, 0.0)))
+        self._ck(self.L.hydro_stage_alpha(self.h, s, 0 if alpha is None else 1, a), "hydro_stage_alpha")
+        return [a[0], a[1], a[2]]
+
+    def stage_sweeps(self, s):
+        self._ck(self.L.hydro_stage_sweeps(self.h, s), "hydro_stage_sweeps")
+
+    def halo(self, s, side, unpack, buf):
+        """buf: CUDA torch tensor of halo_reals() elements of the handle's dtype."""
+        assert buf.is_cuda and buf.is_contiguous() and buf.numel() >= self.halo_reals()
+        self._ck(self.L.hydro_halo(self.h, s, side, 1 if unpack else 0, C.c_void_p(buf.data_ptr())), "hydro_halo")
+
+    def halo_reals(self):
+        return self.L.hydro_halo_reals(self.h)
 
     def set_limiter(self, on=True):
         self._ck(self.L.hydro_set_limiter(self.h, 1 if on else 0), "hydro_set_limiter")

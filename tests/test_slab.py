@@ -1,0 +1,143 @@
+"""z-slab decomposition.  CPU: the plane split, the local extents and the torch.distributed exchange
+over gloo (world_size 3).  GPU (one device): all slabs in one process, exchanged by device copies, against the
+one-handle run -- owned planes must come out bitwise identical."""
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+
+from paper_1511_02137_b200 import slab as SL
+from paper_1511_02137_b200 import synthetic as S
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_split_and_extents():
+    assert SL.split_planes(10, 2) == [(0, 5), (5, 10)]
+    assert SL.split_planes(14, 3) == [(0, 5), (5, 10), (10, 14)]
+    with pytest.raises(ValueError):
+        SL.split_planes(7, 2)
+    for nz, world in ((32, 2), (33, 3), (64, 5), (16, 4)):
+        covered = []
+        for r in range(world):
+            k_off, nloc, lo, hi = SL.local_extent(nz, world, r)
+            assert k_off >= 0 and k_off + nloc <= nz and hi - lo >= SL.HALO
+            assert lo == (SL.HALO if r > 0 else 0) and nloc - hi == (SL.HALO if r < world - 1 else 0)
+            covered += list(range(k_off + lo, k_off + hi))
+        assert covered == list(range(nz))
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _worker(rank, world, port, q):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    import torch
+    import torch.distributed as dist
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    send = [torch.full((6,), 10.0 * rank + side, dtype=torch.float64) for side in (0, 1)]
+    recv = [torch.full((6,), -1.0, dtype=torch.float64) for _ in (0, 1)]
+    SL.exchange_faces(send, recv, rank, world, dist)
+    amax = SL.allreduce_max([0.1 * rank, 0.5 - 0.1 * rank, 0.3], dist)
+    q.put((rank, recv[0][0].item(), recv[1][0].item(), amax))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_exchange_and_alpha_over_gloo_world3():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    world = 3
+    ps = [ctx.Process(target=_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in ps:
+        p.start()
+    res = sorted(q.get(timeout=180) for _ in ps)
+    for p in ps:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for rank, lo, hi, amax in res:
+        assert lo == (10.0 * (rank - 1) + 1 if rank > 0 else -1.0)          # the lower neighbour's HIGH face
+        assert hi == (10.0 * (rank + 1) + 0 if rank < world - 1 else -1.0)   # the upper neighbour's LOW face
+        assert amax == pytest.approx([0.2, 0.5, 0.3])
+
+
+# ------------------------------------------------------------------------------------------------ one GPU, all slabs
+@pytest.fixture(scope="module")
+def H():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_1511_02137_b200 import hydro
+    hydro.load()
+    return hydro
+
+
+CASES = [
+    dict(n=(32, 24, 40), world=2, steps=4, jets=[((-0.5, 0.0, 0.02), (1.0, 0.2, 0.3))]),
+    dict(n=(36, 20, 33), world=3, steps=3, jets=[((0.0, 0.0, 0.0), (0.0, 0.0, 1.0)), ((0.3, 0.1, -0.6), (0.0, 0.0, -1.0))]),
+    dict(n=(32, 24, 40), world=2, steps=3, jets=[((-0.5, 0.0, 0.02), (1.0, 0.2, 0.3))], limiter=True),
+    dict(n=(32, 24, 40), world=2, steps=3, jets=[((-0.5, 0.0, 0.35), (0.0, 0.0, 1.0))], sigma=0.1),
+    dict(n=(32, 24, 40), world=4, steps=3, jets=[((-0.5, 0.0, 0.02), (1.0, 0.2, 0.3))], precision=32),
+    dict(n=(32, 24, 40), world=2, steps=3, jets=[((-0.5, 0.0, 0.02), (1.0, 0.2, 0.3))], weno_order=5, nf=5),
+]
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("case", CASES)
+def test_slabs_match_the_single_handle_run_bitwise(H, case):
+    n, world, steps = case["n"], case["world"], case["steps"]
+    c = S.scaled_config(0, n)
+    c["nf"] = case.get("nf", 4)
+    kw = dict(nfields=c["nf"], precision=case.get("precision", 64), weno_order=case.get("weno_order", 7))
+    U0 = S.make_state(c).astype(np.float64 if kw["precision"] == 64 else np.float32)
+
+    def setup(g):
+        for pos, d in case["jets"]:
+            g.add_jet(pos, d)
+        if case.get("limiter"):
+            g.set_limiter(True)
+        g.set_deposit_width(case.get("sigma", 0.0))
+
+    ref = H.Hydro(*n, c["dx"], c["dt"], **kw)
+    ref.set_state(U0)
+    setup(ref)
+    ref.step(steps)
+    Uref, dref, qref = ref.get_fields(), ref.diag(), ref.last_stage_q()
+
+    slabs = [SL.Slab(H, n, c["dx"], c["dt"], r, world, **kw) for r in range(world)]
+    for sl in slabs:
+        sl.set_state(U0)
+        setup(sl.g)
+    SL.run_local(slabs, steps)
+    U = np.concatenate([sl.owned() for sl in slabs], axis=1)
+    assert U.shape == Uref.shape
+    assert np.array_equal(U, Uref)                                              # bitwise
+    ds = [sl.g.diag() for sl in slabs]
+    assert all(d["step"] == steps and d["has_nan"] == 0 for d in ds)
+    assert sum(d["ncap"] for d in ds) == dref["ncap"]
+    assert np.allclose(sum(d["deposited"] for d in ds), dref["deposited"], rtol=1e-13, atol=0)
+    assert np.allclose(sum(sl.g.last_stage_q() for sl in slabs), qref, rtol=1e-13, atol=0)
+    assert np.array_equal(np.max([d["alpha"] for d in ds], axis=0), dref["alpha"])
+    for sl in slabs:
+        sl.close()
+    ref.close()
+
+
+@pytest.mark.gpu
+def test_slab_argument_checks(H):
+    g = H.Hydro(16, 16, 12, 0.1, 0.02)
+    with pytest.raises(H.HydroError):
+        g.set_slab(32, 8, 2, 8)          # an interior low end needs 4 halo planes
+    with pytest.raises(H.HydroError):
+        g.set_slab(8, 0, 0, 12)          # local array larger than the grid
+    g.set_slab(32, 8, 4, 8)
+    g.close()
