@@ -388,20 +388,55 @@ struct SweepCtx {
     //   F^d_E = M_d;  F^d_{M_j} = M_j v_d + p delta_jd;  F^d_{N_B} = N_B v_d;  v_d = M_d * W   (a-3)
     // written branch-free as F = A * B + C with per-warp operand tiles: energy A = M_d, B = 1, C = 0;
     // momenta / N_B: A = U_f, B = M_d W, C = p (normal component) or 0.
+    struct RowIn { R u, md, w, a, p; };
+    template <int r>
+    __device__ __forceinline__ void load(RowIn& in) const {
+        in.u = pu.template at<r>();
+        in.md = pmd.template at<r>();
+        in.w = pw.template at<r>();
+        in.a = pa.template at<r>();
+        in.p = pp.template at<r>();
+    }
+    template <int r>
+    __device__ __forceinline__ void push(const RowIn& in) {
+        typedef Real<R> T;
+        const R B = T::fma_(in.md, in.w, kE);
+        const R F = T::fma_(in.a, B, in.p);
+        rot_push<r, ORDER, R>(wp, T::fma_(alpha, in.u, F), c3, eps);
+        rot_push<r, ORDER, R>(wm, T::fma_(-alpha, in.u, F), c3, eps);
+    }
     template <int r>
     __device__ __forceinline__ void load_push() {
-        typedef Real<R> T;
-        const R u = pu.template at<r>();
-        const R md = pmd.template at<r>();
-        const R B = T::fma_(md, pw.template at<r>(), kE);
-        const R F = T::fma_(pa.template at<r>(), B, pp.template at<r>());
-        rot_push<r, ORDER, R>(wp, T::fma_(alpha, u, F), c3, eps);
-        rot_push<r, ORDER, R>(wm, T::fma_(-alpha, u, F), c3, eps);
+        RowIn in;
+        load<r>(in);
+        push<r>(in);
+    }
+    // The 8 rows of a chunk, software-pipelined by hand: the shared-memory loads of row r+1 are issued BEFORE row r
+    // is emitted -- the compiler cannot move a load above the output-tile store (it cannot prove they do not alias), so
+    // in source order "load, compute, store" per row every row would start with an exposed load latency and end with
+    // the serial reciprocal chain.  MODE 0: emit<r>(); MODE 1: limiter phase A (corr_store).
+    template <int MODE, int r>
+    __device__ __forceinline__ void tail(const RowIn& in) {
+        push<r>(in);
+        if (MODE == 0) emit<r>();
+        else corr_tail<r>();
+    }
+    template <int MODE>
+    __device__ __forceinline__ void rows() {
+        RowIn i0, i1;
+        load<0>(i0);
+        load<1>(i1); tail<MODE, 0>(i0);
+        load<2>(i0); tail<MODE, 1>(i1);
+        load<3>(i1); tail<MODE, 2>(i0);
+        load<4>(i0); tail<MODE, 3>(i1);
+        load<5>(i1); tail<MODE, 4>(i0);
+        load<6>(i0); tail<MODE, 5>(i1);
+        load<7>(i1); tail<MODE, 6>(i0);
+        tail<MODE, 7>(i1);
     }
     // limiter, phase A: the row's high-order correction goes to the exchange tile
     template <int r>
-    __device__ __forceinline__ void corr_store() {
-        load_push<r>();
+    __device__ __forceinline__ void corr_tail() {
         R vsum, corr;
         rot_flux_parts<r, ORDER, R>(wp, wm, eps, vsum, corr);
         xc_own[sub_off<DIR, R>(r, lane)] = corr;
@@ -430,11 +465,6 @@ struct SweepCtx {
             if (OUT == OUT_COMBINE) o = T::fma_(rk_b, o, rk_a * pun.template at<r>());
         }
         out[sub_off<DIR, R>(r, lane)] = o;
-    }
-    template <int r>
-    __device__ __forceinline__ void row() {
-        load_push<r>();
-        emit<r>();
     }
 };
 
@@ -595,12 +625,10 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
                 cx.fhat_prev = tht[sub_off<DIR, R>(7, lane)] * corr;
             }
         } else if (!LIM) {
-            cx.template row<0>(); cx.template row<1>(); cx.template row<2>(); cx.template row<3>();
-            cx.template row<4>(); cx.template row<5>(); cx.template row<6>(); cx.template row<7>();
+            cx.template rows<0>();
         } else {
             // R16: (A) corrections of all fields to shared memory, (B) one theta per face from all fields, (C) emit
-            cx.template corr_store<0>(); cx.template corr_store<1>(); cx.template corr_store<2>(); cx.template corr_store<3>();
-            cx.template corr_store<4>(); cx.template corr_store<5>(); cx.template corr_store<6>(); cx.template corr_store<7>();
+            cx.template rows<1>();
             __syncthreads();
             const R k3 = (R)a.k3lam;
             switch (f) {
