@@ -316,10 +316,16 @@ int eval_stage_ring(hydro* h, const void* Uin, int slot, int stage, double stage
         la.U = (const R*)Uin; la.P = (const R*)h->P; la.W = (const R*)h->W; la.UL = (R*)h->L; la.diag = h->diag; la.slot = slot;
         la.nx = h->nx; la.ny = h->ny; la.nz = h->nz; la.nxp = h->nxp; la.nf = h->nf; la.N = h->N; la.Np = h->Np;
         la.lam = (R)(h->dt / h->dx);
-        if (h->ny > 65535 || h->nz > 65535) return HYDRO_EINVAL;
         {
+            const long long cols = (long long)((h->nx + 31) / 32) * ((h->ny + 7) / 8);
+            int segs = 1;                                               // z segments: enough blocks to fill the machine
+            while (cols * segs < (long long)h->num_sms * 8 && h->nz / (segs * 2) >= 8) segs *= 2;
+            const int seg_len = (h->nz + segs - 1) / segs;
+            if ((h->ny + 7) / 8 > 65535) return HYDRO_EINVAL;
             Timer t(h, HYDRO_K_PRIM);
-            k_lowup<R><<<dim3((unsigned)((h->nx + 127) / 128), (unsigned)h->ny, (unsigned)h->nz), 128, 0, h->stream>>>(la);
+            const dim3 grid((unsigned)((h->nx + 31) / 32), (unsigned)((h->ny + 7) / 8), (unsigned)((h->nz + seg_len - 1) / seg_len));
+            if (h->nf == 4) k_lowup<R, 4><<<grid, dim3(32, 8, 1), 0, h->stream>>>(la, seg_len);
+            else k_lowup<R, 5><<<grid, dim3(32, 8, 1), 0, h->stream>>>(la, seg_len);
         }
         h->launches += 1;
         CK(cudaGetLastError());

@@ -255,7 +255,6 @@ __global__ void __launch_bounds__(256) k_prims_out(const R* __restrict__ U, R* _
 // ------------------------------------------------------------------------------------------------ limiter: U^L (R16, f-1)
 // First-order Lax-Friedrichs update  U^L = U - (dt/dx) sum_d (F^L_{i+1/2} - F^L_{i-1/2}),
 // F^L_{i+1/2} = [(F_i + alpha U_i) + (F_{i+1} - alpha U_{i+1})] / 2, neighbours clamped (zero-gradient ghosts).
-// One thread per cell, all fields; the 6 neighbours come through L1/L2.  Launch: grid (ceil(nx/128), ny, nz) x 128.
 template <typename R>
 struct LowArgs {
     const R* U; const R* P; const R* W; R* UL;
@@ -265,37 +264,62 @@ struct LowArgs {
     R lam;                       // dt / dx
 };
 
-template <typename R>
-__global__ void __launch_bounds__(128) k_lowup(LowArgs<R> a) {
+// Launch: block (32, 8) = a tile of 32 x 8 columns, grid (ceil(nx/32), ceil(ny/8), z segments); every thread marches its
+// column along z keeping the cell below / at / above in registers (the z neighbours cost no loads); the four in-plane
+// neighbours are L1 hits (they are the plane the block's own threads loaded one trip earlier).
+template <typename R, int NF>
+struct LowCell { R u[NF], w, p; };
+
+template <typename R, int NF>
+__device__ __forceinline__ void low_load(const LowArgs<R>& a, long long c, LowCell<R, NF>& x) {
+#pragma unroll
+    for (int q = 0; q < NF; ++q) x.u[q] = a.U[q * a.Np + c];
+    x.w = a.W[c];
+    x.p = a.P[c];
+}
+// (F^d_q - s alpha U_q) of a cell, s = +1 (upper neighbour) or -1 (lower neighbour)
+template <typename R, int NF>
+__device__ __forceinline__ R low_term(const LowCell<R, NF>& x, int d, int q, R s_alpha) {
+    R F;
+    if (q == 0) F = x.u[1 + d];
+    else {
+        F = x.u[q] * (x.u[1 + d] * x.w);
+        if (q == 1 + d) F += x.p;
+    }
+    return F - s_alpha * x.u[q];
+}
+
+template <typename R, int NF>
+__global__ void __launch_bounds__(256) k_lowup(LowArgs<R> a, int seg_len) {
     typedef Real<R> T;
     R alpha[3];
 #pragma unroll
     for (int d = 0; d < 3; ++d) alpha[d] = T::from_bits(a.diag->slot[a.slot].alpha_bits[d]);
-    // grid = (x tiles, ny, nz): no integer division per cell
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
-    if (i < a.nx) {
-        const long long c = ((long long)k * a.ny + j) * a.nxp + i;
-        R acc[5], Uc[5];
-        for (int q = 0; q < a.nf; ++q) { Uc[q] = a.U[q * a.Np + c]; acc[q] = R(0); }
-#pragma unroll
-        for (int d = 0; d < 3; ++d) {
-            const int id = d == 0 ? i : d == 1 ? j : k, nd = d == 0 ? a.nx : d == 1 ? a.ny : a.nz;
-            const long long st = d == 0 ? 1 : d == 1 ? a.nxp : (long long)a.nxp * a.ny;
-            const long long cm = id > 0 ? c - st : c, cp = id < nd - 1 ? c + st : c;
-            // sum over the two faces: (F^L_+ - F^L_-) = [ (F_p - alpha U_p) - (F_m + alpha U_m) ] / 2 + alpha U_c
-            const R vdp = a.U[(1 + d) * a.Np + cp] * a.W[cp], vdm = a.U[(1 + d) * a.Np + cm] * a.W[cm];
-            for (int q = 0; q < a.nf; ++q) {
-                const R up = a.U[q * a.Np + cp], um = a.U[q * a.Np + cm];
-                R Fp, Fm;
-                if (q == 0) { Fp = a.U[(1 + d) * a.Np + cp]; Fm = a.U[(1 + d) * a.Np + cm]; }
-                else {
-                    Fp = up * vdp; Fm = um * vdm;
-                    if (q == 1 + d) { Fp += a.P[cp]; Fm += a.P[cm]; }
-                }
-                acc[q] += R(0.5) * ((Fp - alpha[d] * up) - (Fm + alpha[d] * um)) + alpha[d] * Uc[q];
-            }
-        }
-        for (int q = 0; q < a.nf; ++q) a.UL[q * a.Np + c] = T::fma_(-a.lam, acc[q], Uc[q]);
+    const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y;
+    const int k0 = blockIdx.z * seg_len, k1 = min(a.nz, k0 + seg_len);
+    if (i >= a.nx || j >= a.ny || k0 >= k1) return;
+    const long long sx = 1, sy = a.nxp, sz = (long long)a.nxp * a.ny;
+    long long c = ((long long)k0 * a.ny + j) * a.nxp + i;
+    LowCell<R, NF> below, here, above, nb;
+    low_load<R, NF>(a, c, here);
+    low_load<R, NF>(a, k0 > 0 ? c - sz : c, below);
+    for (int k = k0; k < k1; ++k, c += sz) {
+        low_load<R, NF>(a, k < a.nz - 1 ? c + sz : c, above);
+        R acc[NF];
+        // sum over the two faces of a direction: (F^L_+ - F^L_-) = [ (F_p - alpha U_p) - (F_m + alpha U_m) ] / 2 + alpha U_c
+        _Pragma("unroll") for (int q = 0; q < NF; ++q)
+            acc[q] = R(0.5) * (low_term<R, NF>(above, 2, q, alpha[2]) - low_term<R, NF>(below, 2, q, -alpha[2])) + alpha[2] * here.u[q];
+        low_load<R, NF>(a, i < a.nx - 1 ? c + sx : c, nb);
+        _Pragma("unroll") for (int q = 0; q < NF; ++q) acc[q] += R(0.5) * low_term<R, NF>(nb, 0, q, alpha[0]) + alpha[0] * here.u[q];
+        low_load<R, NF>(a, i > 0 ? c - sx : c, nb);
+        _Pragma("unroll") for (int q = 0; q < NF; ++q) acc[q] -= R(0.5) * low_term<R, NF>(nb, 0, q, -alpha[0]);
+        low_load<R, NF>(a, j < a.ny - 1 ? c + sy : c, nb);
+        _Pragma("unroll") for (int q = 0; q < NF; ++q) acc[q] += R(0.5) * low_term<R, NF>(nb, 1, q, alpha[1]) + alpha[1] * here.u[q];
+        low_load<R, NF>(a, j > 0 ? c - sy : c, nb);
+        _Pragma("unroll") for (int q = 0; q < NF; ++q) acc[q] -= R(0.5) * low_term<R, NF>(nb, 1, q, -alpha[1]);
+        _Pragma("unroll") for (int q = 0; q < NF; ++q) a.UL[q * a.Np + c] = T::fma_(-a.lam, acc[q], here.u[q]);
+        below = here;
+        here = above;
     }
 }
 
