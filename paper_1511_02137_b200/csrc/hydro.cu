@@ -624,10 +624,8 @@ int hydro_stage_alpha(hydro_t* h, int s, int set, double alpha[3]) {
 
 int hydro_halo(hydro_t* h, int s, int side, int unpack, void* dev_buf) {
     if (!h || s < 0 || s > 2 || (side != 0 && side != 1) || !dev_buf) return HYDRO_EINVAL;
-    const StagePlan p = stage_plan(h, s == 2 ? 2 : s);
-    // stage s's OUTPUT state; after stage 2 the plan has rotated (prim_slot flipped) but buf[cur] is still U^{n+1}
+    // stage s's OUTPUT state (buffer roles are fixed within a handle: buf[cur] = U^n and, after stage 2, U^{n+1})
     char* base = (char*)(s == 0 ? h->buf[(h->cur + 1) % 3] : s == 1 ? h->buf[(h->cur + 2) % 3] : h->buf[h->cur]);
-    (void)p;
     const size_t plane = (size_t)h->nxp * h->ny * h->esz, width = 4 * plane, fpitch = (size_t)h->Np * h->esz;
     int k0;                                   // first of the 4 planes
     if (!unpack) k0 = side == 0 ? h->own_lo : h->own_hi - 4;            // owned boundary planes -> buffer

@@ -48,9 +48,13 @@ def load():
     global _lib
     if _lib is not None:
         return _lib
-    if not os.path.exists(LIB_PATH):
-        raise ImportError("CUDA library %s is missing: run `python -m paper_1511_02137_b200.build` "
-                          "(there is no CPU fallback)" % LIB_PATH)
+    try:                                   # (re)build in-tree if the library is missing or older than its sources
+        from . import build as _build
+        _build.build()
+    except Exception as e:                 # no nvcc, or a compile error: fail loudly below if there is nothing to load
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("CUDA library %s is missing and could not be built (%s): run "
+                              "`python -m paper_1511_02137_b200.build` (there is no CPU fallback)" % (LIB_PATH, e))
     L = C.CDLL(LIB_PATH)
     vp, i, d, ll = C.c_void_p, C.c_int, C.c_double, C.c_longlong
     dp = C.POINTER(C.c_double)

@@ -171,3 +171,17 @@ def test_flop_count_is_measured(oracle):
     assert br["weno7"] == 147            # textbook WENO7-JS with per-weight divisions (SURVEY hand count: 143)
     assert 3500 < tot4 < 4000 and 4400 < tot5 < 5000
     assert abs(tot4 - (br["con2prim"] + br["wavespeeds"] + 3 * (br["interface_flux"] + br["divergence"]) + br["rk"])) < 1e-9
+
+
+def test_bench_flop_constants_are_the_measured_counts(oracle):
+    """bench.py's roofline uses the algorithmic flop counts measured on the oracle's counting type."""
+    import os
+    import sys
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    import bench
+    for nf in (4, 5):
+        for order, tot_tab, sw_tab in ((7, bench.FLOPS_STAGE, bench.FLOPS_SWEEPS_STAGE),
+                                       (5, bench.FLOPS_STAGE_W5, bench.FLOPS_SWEEPS_STAGE_W5)):
+            tot, br = oracle.count_flops(nf, order)
+            assert tot_tab[nf] == tot
+            assert sw_tab[nf] == 3 * (br["interface_flux"] + br["divergence"]) + br["rk"]
