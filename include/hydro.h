@@ -74,6 +74,11 @@ int hydro_set_state(hydro_t *h, const void *U, int memspace);
 int hydro_add_jet(hydro_t *h, double x0, double y0, double z0, double dirx, double diry, double dirz,
                   double kappa_rad, double kappa_coll, double cr_over_cf, int *id);
 int hydro_clear_jets(hydro_t *h);
+
+/* Checkpoint / resume: the state of a run is (U, completed steps, the jets as added).  After hydro_set_state(U of a
+ * checkpoint) and re-adding the jets with their ORIGINAL start positions, hydro_set_step(h, n) restores the step
+ * counter, so that jet positions and path lengths continue from t = n dt; the continuation is bitwise the same run. */
+int hydro_set_step(hydro_t *h, long long step);
 /* ---- z-slab decomposition over several GPUs: one handle per rank -------------------------------
  * The handle's grid is the rank's LOCAL array: its owned planes plus 4 halo planes towards each neighbouring rank (none
  * at a physical boundary, where the zero-gradient ghosts of a-7 act).  hydro_set_slab: nz_global = planes of the whole

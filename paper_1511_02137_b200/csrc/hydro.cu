@@ -661,6 +661,12 @@ int hydro_set_deposit_width(hydro_t* h, double sigma) {
     return HYDRO_OK;
 }
 
+int hydro_set_step(hydro_t* h, long long step) {
+    if (!h || step < 0) return HYDRO_EINVAL;
+    h->step = step;
+    return HYDRO_OK;
+}
+
 int hydro_clear_jets(hydro_t* h) {
     if (!h) return HYDRO_EINVAL;
     h->jets.clear();

@@ -22,7 +22,7 @@ FIELDS_CONSERVED, FIELDS_PRIMITIVE = 0, 1
 K_NAMES = ("prim", "sweep_x", "sweep_y", "sweep_z", "source")
 
 # every symbol include/hydro.h declares (tests check that the library exports all of them)
-SYMBOLS = ("hydro_create", "hydro_destroy", "hydro_set_state", "hydro_add_jet", "hydro_clear_jets", "hydro_set_deposit_width", "hydro_set_limiter", "hydro_get_limited_faces", "hydro_set_slab", "hydro_stage_prims",
+SYMBOLS = ("hydro_create", "hydro_destroy", "hydro_set_state", "hydro_add_jet", "hydro_clear_jets", "hydro_set_step", "hydro_set_deposit_width", "hydro_set_limiter", "hydro_get_limited_faces", "hydro_set_slab", "hydro_stage_prims",
            "hydro_stage_alpha", "hydro_stage_sweeps", "hydro_halo", "hydro_halo_reals", "hydro_step",
            "hydro_synchronize", "hydro_get_fields", "hydro_eval_rhs", "hydro_get_diag", "hydro_get_last_stage_q",
            "hydro_set_profiling", "hydro_get_kernel_times", "hydro_launch_count", "hydro_sweep_path", "hydro_measure_alu_peak",
@@ -68,6 +68,8 @@ def load():
     L.hydro_add_jet.argtypes = [vp] + [d] * 9 + [C.POINTER(i)]
     L.hydro_clear_jets.restype = i
     L.hydro_clear_jets.argtypes = [vp]
+    L.hydro_set_step.restype = i
+    L.hydro_set_step.argtypes = [vp, ll]
     L.hydro_set_slab.restype = i
     L.hydro_set_slab.argtypes = [vp, i, i, i, i]
     L.hydro_stage_prims.restype = i
@@ -199,6 +201,9 @@ class Hydro:
                                       cr_over_cf, C.byref(jid)), "hydro_add_jet")
         self.njets += 1
         return jid.value
+
+    def set_step(self, step):
+        self._ck(self.L.hydro_set_step(self.h, int(step)), "hydro_set_step")
 
     def clear_jets(self):
         self._ck(self.L.hydro_clear_jets(self.h), "hydro_clear_jets")

@@ -575,6 +575,31 @@ def test_device_pointers_and_streams(H, oracle):
     g.close(), g2.close()
 
 
+def test_checkpoint_resume_is_bitwise(H):
+    """(U, step counter, jets) is a complete checkpoint: a run resumed in a NEW handle continues bitwise."""
+    c = S.scaled_config(0, (40, 24, 20))
+    U0 = S.make_state(c)
+    jets = [((-1.0, 0.0, 0.0), (1.0, 0.0, 0.0)), ((0.3, 0.2, -0.1), (0.0, 1.0, 0.5))]
+    g = H.Hydro(*c["n"], c["dx"], c["dt"])
+    g.set_state(U0)
+    for pos, d in jets:
+        g.add_jet(pos, d)
+    g.step(4)
+    Uc, dep_c = g.get_fields(), g.diag()["deposited"]
+    g.step(5)
+    Uref, dref = g.get_fields(), g.diag()
+    r = H.Hydro(*c["n"], c["dx"], c["dt"])
+    r.set_state(Uc)
+    for pos, d in jets:
+        r.add_jet(pos, d)
+    r.set_step(4)
+    r.step(5)
+    assert np.array_equal(r.get_fields(), Uref)
+    dr = r.diag()
+    assert dr["step"] == 9 and np.allclose(dep_c + dr["deposited"], dref["deposited"], rtol=1e-13, atol=0)
+    g.close(), r.close()
+
+
 def test_error_paths(H):
     g = H.Hydro(8, 8, 8, 0.1, 0.02)
     with pytest.raises(H.HydroError):
