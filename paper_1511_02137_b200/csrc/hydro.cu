@@ -24,6 +24,7 @@ struct hydro {
     double dx, dt, weno_eps, delta, e_floor;
     double sigma;                       // Gaussian deposit width [fm]; 0 = point deposit
     int limiter;                        // 1: positivity-preserving flux limiter (R16; fp64 only)
+    bool tail_split;                    // sweeps: short blocks for the partial last wave (HYDRO_NO_TAIL_SPLIT=1 disables)
     int nz_global, k_offset, own_lo, own_hi;   // z-slab decomposition (f-4); defaults: nz, 0, 0, nz
     size_t esz;                         // bytes per real
     cudaStream_t stream;
@@ -159,7 +160,28 @@ int launch_ring_nf(hydro* h, const void* Us, int slot, const CUtensorMap* out_ma
         a.k3lam = 3.0 * h->dt / h->dx; a.nlim = &h->diag->nlim_total;
         const int nlane = DIR == 0 ? h->ny : h->nx;
         const int other = DIR == 2 ? h->ny : h->nz;
-        dim3 grid((unsigned)(((nlane + 31) / 32) * other), (unsigned)h->tma_nseg[DIR], 1);
+        const int nd = DIR == 0 ? h->nx : DIR == 1 ? h->ny : h->nz;
+        const long long tiles = (long long)((nlane + 31) / 32) * other;
+        dim3 grid((unsigned)tiles, (unsigned)h->tma_nseg[DIR], 1);
+        a.n_long = -1; a.short_nseg = 1; a.short_len = nd;
+        // tail splitting: whole-line blocks for the complete waves, short blocks for the partial last wave
+        const long long slots = (long long)h->num_sms * ring_blocks_per_sm(NF, sizeof(R), OUT, LIM);
+        if (h->tail_split && h->tma_nseg[DIR] == 1 && tiles > slots && tiles % slots != 0 && nd >= 64) {
+            const long long n_long = tiles / slots * slots, rem = tiles - n_long;
+            int best_k = 1;
+            double best = 1.0;                                          // cost of the last wave in units of a whole-line wave
+            for (int k = 2; k <= 8 && nd / k >= 32; k *= 2) {
+                const int sl = ((nd + k - 1) / k + RING_CH - 1) / RING_CH * RING_CH;
+                const int kk = (nd + sl - 1) / sl;
+                const double waves = (double)((rem * kk + slots - 1) / slots);
+                const double cost = waves * (sl + RING_CH) / (double)(nd + RING_CH);
+                if (cost < best - 1e-9) { best = cost; best_k = kk; a.short_len = sl; }
+            }
+            if (best_k > 1) {
+                a.n_long = (int)n_long; a.short_nseg = best_k;
+                grid = dim3((unsigned)(n_long + rem * best_k), 1, 1);
+            } else a.short_len = nd;
+        }
         dim3 block(32, NF, 1);
         {
             Timer t(h, HYDRO_K_SWEEP_X + DIR);
@@ -482,6 +504,7 @@ int hydro_create(hydro_t** out, int nx, int ny, int nz, double dx, double dt, co
     h->order = o.weno_order == 5 ? 5 : 7;
     h->sigma = 0.0;
     h->limiter = 0;
+    { const char* ts = getenv("HYDRO_NO_TAIL_SPLIT"); h->tail_split = !(ts && ts[0] == '1'); }
     h->nz_global = nz; h->k_offset = 0; h->own_lo = 0; h->own_hi = nz;
     h->dx = dx; h->dt = dt;
     h->weno_eps = o.weno_eps > 0 ? o.weno_eps : 1e-6;

@@ -121,6 +121,7 @@ struct RingArgs {
     int slot;                  // which DiagSlot holds alpha of U_s
     int nx, ny, nz;
     int seg_len;               // march cells per block (multiple of RING_CH)
+    int n_long, short_nseg, short_len;   // tail-split mode (n_long >= 0), see the kernel
     double eps_eff;            // WENO7: 144 * weno_eps (the split fluxes are carried as 2 f^+-, beta as 36 beta); WENO5: 48 * weno_eps
     double coef;               // OUT_STORE / OUT_REDUCE: c = [b dt] / (2 dx);  OUT_COMBINE*: 1 / (2 dx)
     double dt, rk_a, rk_b;
@@ -488,18 +489,29 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
     const bool leader = (lane == 0 && f == 0);
     const int nd = DIR == 0 ? a.nx : DIR == 1 ? a.ny : a.nz;
 
-    // transverse tile of 32 lines and the march segment of this block
+    // transverse tile of 32 lines and the march segment of this block.  Uniform mode (n_long < 0): blockIdx.x = tile,
+    // blockIdx.y = segment of seg_len cells.  Tail-split mode: the first n_long tiles are marched whole by one block each
+    // (they fill complete waves of resident blocks); the remaining tiles are cut into short_nseg segments of short_len
+    // cells so that the last, partial wave is made of short blocks.
+    int tile, s0, seglen;
+    if (a.n_long < 0) { tile = blockIdx.x; s0 = blockIdx.y * a.seg_len; seglen = a.seg_len; }
+    else if ((int)blockIdx.x < a.n_long) { tile = blockIdx.x; s0 = 0; seglen = nd; }
+    else {
+        const int bb = blockIdx.x - a.n_long;
+        tile = a.n_long + bb / a.short_nseg;
+        s0 = (bb % a.short_nseg) * a.short_len;
+        seglen = a.short_len;
+    }
     int t0, tfix;                  // first transverse index along the lane axis, fixed transverse index
     {
         const int nlane_axis = DIR == 0 ? a.ny : a.nx;
         const int tiles = (nlane_axis + 31) >> 5;
-        const int tb = blockIdx.x % tiles;
-        tfix = blockIdx.x / tiles;
+        const int tb = tile % tiles;
+        tfix = tile / tiles;
         t0 = tb << 5;
     }
-    const int s0 = blockIdx.y * a.seg_len;
     if (s0 >= nd) return;          // whole block exits together
-    const int len = min(nd, s0 + a.seg_len) - s0;
+    const int len = min(nd, s0 + seglen) - s0;
     const int nchunks = (len + RING_CH - 1) / RING_CH + 1;             // chunk m holds cells s0 - 4 + 8m .. + 7
 
     if (leader) {
