@@ -46,8 +46,8 @@ FLOPS_STAGE_W5 = {4: 1820.0, 5: 2261.0}
 FLOPS_SWEEPS_STAGE_W5 = {4: 3 * (560.0 + 12.0) + 20.0, 5: 3 * (700.0 + 15.0) + 25.0}
 FP64_NOMINAL_TF = 148 * 64 * 2 * 1.965e9 / 1e12          # 148 SMs x 64 DFMA/clk x 2 x 1.965 GHz = 37.2
 # dram__bytes_read.sum + dram__bytes_write.sum per sweep launch at 256^3 fp64 nf=4, mean of the x (COMBINE), y and z
-# (REDUCE) kernels, from the one `ncu --set full` capture summarised in profiles/r1_g_ring_ncu_summary.txt
-NCU_TRAFFIC_SWEEP_256_F64_NF4 = (1.310e9 + 1.837e9 + 1.839e9) / 3.0
+# (REDUCE) kernels, from the one `ncu --set full` capture summarised in profiles/r1_i_ring_ncu_summary.txt
+NCU_TRAFFIC_SWEEP_256_F64_NF4 = (1.315e9 + 1.839e9 + 1.841e9) / 3.0
 
 
 def max_over_ranks(values, world, device):
@@ -357,9 +357,9 @@ def main():
                 "share_of_step": sw_ms / all_ms if all_ms else None,
                 "kernel_ms_per_step": {k: v["ms"] / args.steps for k, v in kt.items()},
                 "whole_path_frac": (fl_stage * 3 * value) / (peak_tf * 1e12),
-                "fp64_pipe_busy_ncu": 0.817 if (cfg == 3 and args.precision == 64 and args.weno_order == 7 and not args.limiter) else None,
+                "fp64_pipe_busy_ncu": 0.856 if (cfg == 3 and args.precision == 64 and args.weno_order == 7 and not args.limiter) else None,
                 "traffic": NCU_TRAFFIC_SWEEP_256_F64_NF4 if (cfg == 3 and args.precision == 64 and args.weno_order == 7) else None,
-                "traffic_source": "profiles/r1_g_ring_ncu_summary.txt (ncu --set full, dram read+write per launch)",
+                "traffic_source": "profiles/r1_i_ring_ncu_summary.txt (ncu --set full, dram read+write per launch)",
                 "algorithmic_bytes_per_launch": (nf + 2 + nf + nf * 2.0 / 9.0 + 2.0 / 3.0 * nf) * 8.0 * cells}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

@@ -425,6 +425,13 @@ struct SweepCtx {
     template <int MODE>
     __device__ __forceinline__ void rows() {
         RowIn i0, i1;
+        if (sizeof(R) == 8 && NF == 5) {
+            // nf = 5 in fp64 is compiled for <= 136 registers (3 blocks of 160 threads): the extra live row does not fit
+            load<0>(i0); tail<MODE, 0>(i0); load<1>(i0); tail<MODE, 1>(i0); load<2>(i0); tail<MODE, 2>(i0);
+            load<3>(i0); tail<MODE, 3>(i0); load<4>(i0); tail<MODE, 4>(i0); load<5>(i0); tail<MODE, 5>(i0);
+            load<6>(i0); tail<MODE, 6>(i0); load<7>(i0); tail<MODE, 7>(i0);
+            return;
+        }
         load<0>(i0);
         load<1>(i1); tail<MODE, 0>(i0);
         load<2>(i0); tail<MODE, 1>(i1);

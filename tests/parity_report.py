@@ -6,7 +6,7 @@ Advances the CUDA path and the CPU oracle side by side on a BASELINE config and 
 error per conserved field, the cap-event counts of both sides and the differences of alpha and of the deposited totals.
 The full 120-step config 3 run takes ~8 minutes of oracle time on the B200 box's 16 cores, which is why the default
 GPU suite only compares the first steps (tests/test_gpu_parity.py::test_config3_full_size_first_steps); the record of the
-full run is profiles/r1_h_parity_config3_120steps.txt."""
+full run is profiles/r1_i_parity_config3_120steps.txt."""
 import argparse
 import json
 import os
