@@ -150,7 +150,7 @@ __device__ __forceinline__ long long pad_index(long long c, int nx, int nxp) {
 }
 
 template <typename R>
-__global__ void __launch_bounds__(256) k_prim(PrimArgs<R> a) {
+__global__ void __launch_bounds__(256, 4) k_prim(PrimArgs<R> a) {
     R am[3] = {R(0), R(0), R(0)};
     unsigned int ncap = 0, bad = 0;
     const long long stride = (long long)gridDim.x * blockDim.x;
