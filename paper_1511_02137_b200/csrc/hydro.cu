@@ -34,7 +34,6 @@ struct hydro {
     void* L;                            // right-hand side
     void* P;                            // pressure of the state the primitives were last computed for
     void* W;                            // scale/(E+p) of that state
-    void* scratch;                      // nf*N reals for get_fields(primitive) / eval_rhs staging
     Diag* diag;
     JetDev* jets_dev;
     std::vector<JetDev> jets;
@@ -518,7 +517,7 @@ int hydro_create(hydro_t** out, int nx, int ny, int nz, double dx, double dt, co
     }
     h->stream = (cudaStream_t)cuda_stream; h->own_stream = false;
     for (int b = 0; b < 3; ++b) h->buf[b] = 0;
-    h->cur = 0; h->L = h->P = h->W = h->scratch = 0; h->diag = 0; h->jets_dev = 0;
+    h->cur = 0; h->L = h->P = h->W = 0; h->diag = 0; h->jets_dev = 0;
     h->jets_dirty = false; h->step = 0; h->prim_slot = 0; h->prims_valid = false; h->launches = 0;
     h->profiling = false;
     h->chain_prev = 0;
@@ -566,7 +565,7 @@ void hydro_destroy(hydro_t* h) {
     drain_events(h);
     for (size_t n = 0; n < h->ev_pool.size(); ++n) cudaEventDestroy(h->ev_pool[n]);
     for (int b = 0; b < 3; ++b) cudaFree(h->buf[b]);
-    cudaFree(h->L); cudaFree(h->P); cudaFree(h->W); cudaFree(h->scratch); cudaFree(h->diag); cudaFree(h->jets_dev);
+    cudaFree(h->L); cudaFree(h->P); cudaFree(h->W); cudaFree(h->diag); cudaFree(h->jets_dev);
     if (h->own_stream && h->stream) cudaStreamDestroy(h->stream);
     delete h;
 }
