@@ -9,7 +9,9 @@
  *   Cartesian grid, EOS p = e/3, dx = 0.1 fm, dt = 0.02 fm/c, 256^3               :13, :49
  * for the conserved densities U = (T^00, T^0x, T^0y, T^0z [, N_B]).  Everything the paper leaves open
  * (Lax-Friedrichs splitting, WENO-JS weights, Shu-Osher RK3, outflow ghosts, delta-function deposit, T(e),
- * admissibility cap) follows the readings R1-R14 listed in DESIGN.md.
+ * admissibility cap) follows the readings R1-R14 listed in DESIGN.md.  Optional, off by default: the WENO5 variant
+ * (weno_order = 5), the Gaussian deposit (R15), the positivity-preserving flux limiter (R16), z-slab decomposition
+ * over several GPUs and checkpoint/resume -- DESIGN.md 9 and 11.
  *
  * Conventions
  *   - every function returns an int status (HYDRO_OK = 0); nothing throws or aborts;
