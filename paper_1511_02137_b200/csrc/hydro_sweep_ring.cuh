@@ -87,10 +87,10 @@ __device__ __forceinline__ void tma_wait_all0() { asm volatile("cp.async.bulk.wa
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // shared-memory plan of one launch (host and device agree through these functions); units: reals
-__host__ __device__ constexpr int ring_stage_reals(int nf, int lim = 0) { return (nf + 2 + (lim ? nf : 0)) * RING_SUB; }
+__host__ __device__ constexpr int ring_stage_reals(int nf, int lim = 0) { return (lim ? nf + 2 : nf + 2) * RING_SUB; }
 __host__ __device__ constexpr int ring_smem_bytes(int nf, int out, int esz, int lim = 0) {
-    return (RING_NSTAGE * ring_stage_reals(nf, lim)       // input ring (+ U^L tiles with the limiter)
-            + (lim ? (nf + 1) * RING_SUB : 0)              // limiter: flux-correction tiles of all fields + theta tile
+    return (RING_NSTAGE * ring_stage_reals(nf, lim)       // input ring
+            + (lim ? (2 * nf + 1) * RING_SUB : 0)          // limiter: two U^L tiles (this chunk, previous chunk) + theta tile
             + 2 * nf * RING_SUB                            // two output tiles
             + (out == OUT_COMBINE ? 2 * nf * RING_SUB : 0) // two U^n tiles
             + RING_SUB) * esz                              // one tile of zeros
@@ -104,7 +104,7 @@ __host__ __device__ constexpr int ring_smem_bytes(int nf, int out, int esz, int 
 #endif
 // resident blocks per SM the kernels are compiled for (registers: 65536 / (32 NF threads x blocks))
 __host__ __device__ constexpr int ring_blocks_per_sm(int nf, int esz, int out = OUT_COMBINE, int lim = 0) {
-    if (lim) return nf == 4 ? 2 : 1;                       // 88-104 KB (nf = 4), 106-126 KB (nf = 5) of shared memory
+    if (lim) return (nf == 4 && (out == OUT_REDUCE || out == OUT_STORE)) ? 3 : 2;   // 72 KB / <= 168 registers, else 2
     // nf = 5 in fp64: 3 blocks (<= 136 registers, 64 KB) except the combine kernel with its U^n tiles (84 KB): 2
     return esz == 8 ? (nf == 4 ? RING_F64_BLOCKS : (out != OUT_COMBINE ? 3 : 2)) : (nf == 4 ? RING_F32_BLOCKS : 4);
 }
@@ -338,11 +338,11 @@ __device__ __forceinline__ R theta_cell(const R W0[4], const R a[4], R sgn) {
 }
 
 // theta of the face of chunk row r (between march cells i = cm + r - 4 and i + 1) for this lane: reads the corrections of
-// the four energy-momentum fields from the exchange tiles and U^L of the two cells from the ring (rows r-4, r-3; the
-// previous chunk's stage for negative rows).  Cells outside the grid impose no condition.  Returns 1 if theta < 1.
+// the four energy-momentum fields from the chunk's output tiles (where phase A left them) and U^L of the two cells from
+// the two U^L tiles (rows r-4, r-3; the previous chunk's tile for negative rows).  Cells outside the grid impose no condition.  Returns 1 if theta < 1.
 template <int r, int DIR, int NF, typename R>
 __device__ __forceinline__ int theta_row(const R* st, const R* stp, const R* xc_all, R* th, int lane, int cm, int nd, R k3lam) {
-    constexpr int ULB = NF + 2;
+    constexpr int ULB = 0;             // st / stp: the U^L tiles of this chunk / of the previous chunk
     const int o = sub_off<DIR, R>(r, lane);
     R a[4];
 #pragma unroll
@@ -375,7 +375,6 @@ template <typename R, int ORDER, int LIM, int DIR, int OUT, int NF>
 struct SweepCtx {
     RotWin<R> wp, wm;
     R fhat_prev;
-    R* xc_own;                             // limiter: this field's flux-correction tile
     const R* th;                           // limiter: theta tile
     R alpha, c3, eps, coef, dt, rk_a, rk_b, kE;
     // current chunk
@@ -447,13 +446,13 @@ struct SweepCtx {
     __device__ __forceinline__ void corr_tail() {
         R vsum, corr;
         rot_flux_parts<r, ORDER, R>(wp, wm, eps, vsum, corr);
-        xc_own[sub_off<DIR, R>(r, lane)] = corr;
+        out[sub_off<DIR, R>(r, lane)] = corr;                // phase A leaves the correction where the output will go
     }
     // limiter, phase C: the first-order part of every flux is already inside U^L; what is left is theta * corr
     template <int r>
     __device__ __forceinline__ void emit_lim() {
         const int o = sub_off<DIR, R>(r, lane);
-        emit_with<r>(th[o] * xc_own[o]);
+        emit_with<r>(th[o] * out[o]);
     }
     template <int r>
     __device__ __forceinline__ void emit() {
@@ -488,9 +487,10 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
     R* outt = stages + RING_NSTAGE * STAGE_REALS;                      // two output tiles of NF sub-tiles
     R* unt = outt + 2 * NF * RING_SUB;                                 // OUT_COMBINE: two U^n tiles
     R* zeros = unt + (OUT == OUT_COMBINE ? 2 * NF * RING_SUB : 0);
-    R* xc = zeros + RING_SUB;                                          // limiter: NF correction tiles, then the theta tile
-    R* tht = xc + (LIM ? NF * RING_SUB : 0);
+    R* ult = zeros + RING_SUB;                                         // limiter: two U^L tiles of NF sub-tiles, then the theta tile
+    R* tht = ult + (LIM ? 2 * NF * RING_SUB : 0);
     uint64_t* full = (uint64_t*)(tht + (LIM ? RING_SUB : 0));
+    uint64_t* full_ul = full + RING_NSTAGE;
 
     const int lane = threadIdx.x, f = threadIdx.y;
     const bool leader = (lane == 0 && f == 0);
@@ -524,6 +524,7 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
     if (leader) {
 #pragma unroll
         for (int s = 0; s < RING_NSTAGE; ++s) mbar_init(&full[s], 1);
+        if (LIM) { mbar_init(&full_ul[0], 1); mbar_init(&full_ul[1], 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int i = f * 32 + lane; i < RING_SUB; i += 32 * NF) zeros[i] = R(0);
@@ -544,11 +545,16 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
         tma_load_4d(dst, &maps.U, &full[st], c0, c1, c2, 0);
         tma_load_4d(dst + NF * RING_SUB, &maps.W, &full[st], c0, c1, c2, 0);
         tma_load_4d(dst + (NF + 1) * RING_SUB, &maps.P, &full[st], c0, c1, c2, 0);
-        if (LIM) tma_load_4d(dst + (NF + 2) * RING_SUB, &maps.UL, &full[st], c0, c1, c2, 0);
         if (with_un) {
             coords(s0 + (m - 1) * RING_CH, c0, c1, c2);                // the cells chunk m emits
             tma_load_4d(unt + (m & 1) * NF * RING_SUB, &maps.Un, &full[st], c0, c1, c2, 0);
         }
+    };
+    auto issue_ul = [&](int m) {                                       // leader only (limiter): U^L of chunk m's cells
+        int c0, c1, c2;
+        coords(s0 - 4 + m * RING_CH, c0, c1, c2);
+        mbar_expect_tx(&full_ul[m & 1], UN_BYTES);
+        tma_load_4d(ult + (m & 1) * NF * RING_SUB, &maps.UL, &full_ul[m & 1], c0, c1, c2, 0);
     };
     auto flush = [&](int m) {                                          // leader only: write back chunk m's outputs
         int c0, c1, c2;
@@ -561,10 +567,10 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
     if (leader) {
         issue(0);
         if (nchunks > 1) issue(1);
+        if (LIM) issue_ul(0);
     }
 
     SweepCtx<R, ORDER, LIM, DIR, OUT, NF> cx;
-    cx.xc_own = xc + f * RING_SUB;
     cx.th = tht;
     int nlim_local = 0;
     cx.wp.clear();
@@ -590,6 +596,7 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
             if (leader) {
                 if (m > 1) flush(m - 1);
                 if (m + 1 < nchunks) issue(m + 1);                     // overwrites chunk m-2
+                if (LIM) issue_ul(m);                                  // overwrites chunk m-2's U^L (phase B of m-1 is over)
             }
         }
         R* st = stages + (m % RING_NSTAGE) * STAGE_REALS;
@@ -620,12 +627,15 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
         cx.pw.set(is_energy ? zeros : st + NF * RING_SUB, lane);
         cx.pp.set(is_normal ? st + (NF + 1) * RING_SUB : zeros, lane);
         if (OUT == OUT_COMBINE1 || OUT == OUT_COMBINE) {           // the state the stage's own part is added to: U_s, or U^L
-            cx.pus[0].set(stp + (LIM ? NF + 2 + f : f) * RING_SUB, lane);
-            cx.pus[1].set(st + (LIM ? NF + 2 + f : f) * RING_SUB, lane);
+            cx.pus[0].set(LIM ? ult + ((m + 1) & 1) * NF * RING_SUB + f * RING_SUB : stp + f * RING_SUB, lane);
+            cx.pus[1].set(LIM ? ult + (m & 1) * NF * RING_SUB + f * RING_SUB : st + f * RING_SUB, lane);
         }
         if (OUT == OUT_COMBINE) cx.pun.set(unt + (m & 1) * NF * RING_SUB + f * RING_SUB, lane);
         cx.out = outt + (m & 1) * NF * RING_SUB + f * RING_SUB;
 
+        const R* ul_cur = ult + (m & 1) * NF * RING_SUB;            // limiter: U^L tiles of this / the previous chunk
+        const R* ul_prev = ult + ((m + 1) & 1) * NF * RING_SUB;
+        const R* xcm = outt + (m & 1) * NF * RING_SUB;              // limiter: the corrections sit in the output tiles
         if (m == 0) {
             // warm-up chunk: cells s0-4 .. s0+3 fill both windows; the last row gives the interface s0 - 1/2
             cx.template load_push<0>(); cx.template load_push<1>(); cx.template load_push<2>(); cx.template load_push<3>();
@@ -634,10 +644,11 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
             else {
                 R vsum, corr;
                 rot_flux_parts<7, ORDER, R>(cx.wp, cx.wm, cx.eps, vsum, corr);
-                cx.xc_own[sub_off<DIR, R>(7, lane)] = corr;
+                cx.out[sub_off<DIR, R>(7, lane)] = corr;
+                mbar_wait(&full_ul[m & 1], (m >> 1) & 1);
                 __syncthreads();
                 if (f == 0) {
-                    const int n1 = theta_row<7, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, (R)a.k3lam);
+                    const int n1 = theta_row<7, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, (R)a.k3lam);
                     if (s0 == 0) nlim_local += n1;                     // inner segment starts are counted by the segment before
                 }
                 __syncthreads();
@@ -648,17 +659,18 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
         } else {
             // R16: (A) corrections of all fields to shared memory, (B) one theta per face from all fields, (C) emit
             cx.template rows<1>();
+            mbar_wait(&full_ul[m & 1], (m >> 1) & 1);
             __syncthreads();
             const R k3 = (R)a.k3lam;
             switch (f) {
-                case 0: nlim_local += theta_row<0, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, k3) +
-                                      theta_row<1, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, k3); break;
-                case 1: nlim_local += theta_row<2, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, k3) +
-                                      theta_row<3, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, k3); break;
-                case 2: nlim_local += theta_row<4, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, k3) +
-                                      theta_row<5, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, k3); break;
-                case 3: nlim_local += theta_row<6, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, k3) +
-                                      theta_row<7, DIR, NF, R>(st, stp, xc, tht, lane, cm, nd, k3); break;
+                case 0: nlim_local += theta_row<0, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3) +
+                                      theta_row<1, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3); break;
+                case 1: nlim_local += theta_row<2, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3) +
+                                      theta_row<3, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3); break;
+                case 2: nlim_local += theta_row<4, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3) +
+                                      theta_row<5, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3); break;
+                case 3: nlim_local += theta_row<6, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3) +
+                                      theta_row<7, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3); break;
                 default: break;
             }
             __syncthreads();
