@@ -20,11 +20,15 @@
 //  (each cell's arithmetic is unchanged; the only reduction is an exact max / integer sum).
 //
 //  Pins (tests/test_oracle_*.py, -m "not gpu"): P1 con2prim round trip, P2 uniform state
-//  bitwise, P3 WENO7 exactness/order/weights, P4 exact Riemann solution, P5 discrete
-//  conservation + jet budget, P6 mirror symmetry, P7 dimensional embedding/permutation,
-//  P8 source-law values.  The readings R2,R3,R4,R7,R9 themselves cannot be pinned by any
-//  number printed in the paper (it prints none): "parity unpinned against the paper" for those
-//  choices; they are fixed by DESIGN.md only.
+//  bitwise, P3 WENO7 exactness/order/weights (incl. the weight ratios from the integral-definition
+//  beta: exponent 2, absolute eps), P4 exact Riemann solution, P5 discrete conservation + jet
+//  budget, P6 mirror symmetry, P7 dimensional embedding/permutation, P8 source-law values and the
+//  source's stage times t_n, t_n+dt, t_n+dt/2 inside rk3_step (quadrature pin: a frozen-T jet is
+//  integrated exactly).  The limiter (R16): admissibility properties, and its two constants (the
+//  face multiplier 6 and delta = min(1e-8 E, g)) by the exact 1-D case where g is linear.
+//  PARITY UNPINNED against the paper: the readings R2, R3, R4, R7, R9, R15, R16 are choices no
+//  number printed in the paper can distinguish (it prints none); the pins above check that the code
+//  implements the readings as DESIGN.md states them, not that the paper meant them.
 //
 //  Build: g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC hydro_oracle.cpp -o liboracle.so
 // ============================================================================================

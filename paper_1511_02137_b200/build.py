@@ -35,7 +35,8 @@ def build(force=False, verbose=False):
         sys.stderr.write(r.stdout)
     if r.returncode != 0:
         raise RuntimeError("nvcc failed: " + " ".join(cmd))
-    with open(os.path.join(HERE, "libhydro.ptxas.log"), "w") as f:
+    os.makedirs(os.path.join(HERE, "build"), exist_ok=True)               # git-ignored: ptxas -v register / spill report
+    with open(os.path.join(HERE, "build", "libhydro.ptxas.log"), "w") as f:
         f.write(" ".join(cmd) + "\n" + r.stdout)
     os.replace(tmp, LIB)
     return LIB

@@ -824,7 +824,7 @@ const char* hydro_strerror(int code) {
         case HYDRO_EINVAL: return "invalid argument";
         case HYDRO_ENOMEM: return "out of device memory";
         case HYDRO_ECUDA: return "CUDA error (see hydro_last_cuda_error)";
-        case HYDRO_ESTATE: return "invalid state (too many jets)";
+        case HYDRO_ESTATE: return "invalid state for this call (jet table full, buffer not owned by the handle, or option not available in this precision)";
         default: return "unknown error";
     }
 }

@@ -283,7 +283,7 @@ def test_config3_long_run_properties(H):
 @pytest.mark.parametrize("n", [(32, 32, 32), (36, 19, 23), (8, 5, 3), (132, 9, 6), (33, 20, 17), (64, 40, 72)])
 @pytest.mark.parametrize("nf", [4, 5])
 def test_fp32_rhs_single_stage(H, oracle, n, nf):
-    """fp32 variant, one evaluation of L(U): ring kernels when nx % 4 == 0, generic kernels otherwise (R10)."""
+    """fp32 variant, one evaluation of L(U) (R10); every nx runs the ring kernels (rows are pitched to 16 bytes)."""
     c = S.scaled_config(0, n)
     c["nf"] = nf
     c["jets"] = [((-0.12, 0.03, 0.0), (1.0, 0.5, -0.25))]

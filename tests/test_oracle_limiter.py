@@ -121,3 +121,106 @@ def test_conservation_with_limiter_active(oracle):
         s0, s1 = U0[f].sum(dtype=np.longdouble), U[f].sum(dtype=np.longdouble)
         assert abs(float(s1 - s0)) < 1e-11 * float(np.abs(U0[f]).sum())
     o.close()
+
+
+# ------------------------------------------------------------------ R16's constants: exact case with a linear g
+def _weno7_from_definition(v, eps):
+    """WENO7-JS value at the right face of the centre cell from 7 cell values, straight from the definition (O5):
+    cubic p_k with the prescribed cell averages on sub-stencil k (4x4 linear solve), q_k = p_k(face),
+    beta_k = sum_l int_cell dx^(2l-1) (d^l p_k)^2, weights d_k/(eps + beta_k)^2, d = (1, 12, 18, 4)/35."""
+    from numpy.polynomial import polynomial as Pl
+    d = np.array([1.0, 12.0, 18.0, 4.0]) / 35.0
+    q, beta = np.zeros(4), np.zeros(4)
+    for k in range(4):
+        A = np.array([[((r + 0.5) ** (c + 1) - (r - 0.5) ** (c + 1)) / (c + 1) for c in range(4)] for r in range(4)])
+        coef = np.linalg.solve(A, v[k:k + 4])              # unit cells at 0..3; the centre cell sits at 3 - k
+        pos = 3 - k
+        q[k] = Pl.polyval(pos + 0.5, coef)
+        for l in (1, 2, 3):
+            dl = Pl.polyder(coef, l)
+            sq = Pl.polyint(Pl.polymul(dl, dl))
+            beta[k] += Pl.polyval(pos + 0.5, sq) - Pl.polyval(pos - 0.5, sq)
+    a = d / (eps + beta) ** 2
+    return float(a @ q / a.sum())
+
+
+def test_r16_constants_on_a_linear_admissibility_function(oracle):
+    """Reading R16 states: the limited Euler update is the average of the six states
+    W_f = U^L_i -+ 6 (dt/dx) theta_f C_f, and theta_f is the largest value for which g(W_f) >= delta_i =
+    min(1e-8 E^L_i, g(U^L_i)) in both cells of the face, as far as the concavity of g = E - |M| can tell.  In 1-D with
+    momenta along x only, g = E - |M_x| is LINEAR wherever M_x keeps its sign along the segment U^L_i .. W_f(1); there
+    the concavity bound is exact and theta_f is the true supremum, found here by bisection on that definition (no secant
+    formula), with U^L, F^L and the WENO7 fluxes rebuilt from eq. (1), the Lax-Friedrichs splitting and the definition
+    of the reconstruction.  On the remaining limited faces (M_x changes sign: g is only concave) the oracle's theta must
+    be admissible and not larger than the supremum.  The oracle's face fluxes are recovered from its L by summing the
+    divergence from the left boundary, where a uniform pad makes the flux known.  A different face multiplier
+    (6 -> 12) or a different delta (1e-8 -> 1e-4) moves theta on the linear faces and fails this test."""
+    nx, pad, dx, dt, eps = 72, 6, 0.1, 0.02, 1e-6
+    lam = dt / dx
+    rng = np.random.default_rng(3)
+    e = 10.0 ** rng.uniform(-0.5, 0.5, nx)
+    v = rng.uniform(0.6, 0.985, nx)
+    e[:pad], v[:pad] = e[pad], v[pad]                     # uniform pad: the flux through the left boundary is F(U_0)
+    gam2 = 1.0 / (1.0 - v * v)
+    E = (4.0 / 3.0) * e * gam2 - e / 3.0                  # eq. (1), p = e/3
+    M = (4.0 / 3.0) * e * gam2 * v
+    U = np.stack([E, M])                                  # (E, M_x); M_y = M_z = 0 exactly
+    F = np.stack([M, M * v + e / 3.0])                    # F^x = (M_x, M_x v_x + p)
+    cs = 1.0 / np.sqrt(3.0)
+    alpha = np.max((v + cs) / (1.0 + v * cs))             # v > 0: the faster acoustic wave (1-D addition formula)
+    fp, fm = 0.5 * (F + alpha * U), 0.5 * (F - alpha * U)
+    cl = lambda i: min(max(i, 0), nx - 1)                 # zero-gradient ghosts = index clamping (R8b)
+    FH, FL = np.zeros((2, nx + 1)), np.zeros((2, nx + 1))
+    for f in range(nx + 1):                               # face f lies between cells i = f-1 and i+1 = f
+        i = f - 1
+        for q in range(2):
+            wp = np.array([fp[q, cl(i + m)] for m in range(-3, 4)])
+            wm = np.array([fm[q, cl(i + 1 - m)] for m in range(-3, 4)])
+            FH[q, f] = _weno7_from_definition(wp, eps) + _weno7_from_definition(wm, eps)
+            FL[q, f] = fp[q, cl(i)] + fm[q, cl(i + 1)]
+    C = FH - FL
+    UL = U - lam * (FL[:, 1:] - FL[:, :-1])
+    g = lambda W: W[0] - abs(W[1])
+    cells = lambda f: [(c, sgn) for c, sgn in ((f - 1, -1.0), (f, 1.0)) if 0 <= c < nx]
+
+    def admissible(f, t, slack=0.0):
+        return all(g(UL[:, c] + sgn * 6.0 * lam * t * C[:, f]) >= min(1e-8 * UL[0, c], g(UL[:, c])) - slack * UL[0, c]
+                   for c, sgn in cells(f))
+
+    theta, linear = np.ones(nx + 1), np.ones(nx + 1, bool)
+    for f in range(nx + 1):
+        if not admissible(f, 1.0):
+            lo, hi = 0.0, 1.0
+            for _ in range(200):
+                mid = 0.5 * (lo + hi)
+                lo, hi = (mid, hi) if admissible(f, mid) else (lo, mid)
+            theta[f] = lo
+            linear[f] = all(UL[1, c] > 0 and UL[1, c] + sgn * 6.0 * lam * C[1, f] > 0 for c, sgn in cells(f))
+    lim = theta < 1.0
+    assert np.sum(lim & linear & (theta > 0.05) & (theta < 0.95)) >= 4      # the case must exercise the exact regime
+    o = oracle.Oracle(nx, 1, 1, dx, dt)
+    U4 = np.zeros((4, 1, 1, nx))
+    U4[0, 0, 0], U4[1, 0, 0] = E, M
+    o.set_state(U4)
+    o.set_limiter(True)
+    L = o.eval_rhs(0.0)
+    assert abs(o.diag()["alpha"][0] - alpha) < 1e-14
+    assert o.limited_faces() == int(lim.sum())
+    assert np.all(L[2] == 0.0) and np.all(L[3] == 0.0)
+    assert not lim[0] and abs(C[0, 0]) < 1e-13 and abs(C[1, 0]) < 1e-13       # the pad did its job
+    Fo = np.zeros((2, nx + 1))                                                # the oracle's limited face fluxes
+    Fo[:, 0] = FL[:, 0]
+    Fo[:, 1:] = Fo[:, :1] - dx * np.cumsum(L[:2, 0, 0], axis=1)
+    scale = np.max(np.abs(FH), axis=1)
+    for f in range(nx + 1):
+        if not lim[f]:
+            assert np.max(np.abs(Fo[:, f] - FH[:, f]) / scale) < 1e-10, f
+            continue
+        q = int(np.argmax(np.abs(C[:, f]) / scale))
+        th_o = (Fo[q, f] - FL[q, f]) / C[q, f]                               # one theta for all fields
+        assert np.max(np.abs(Fo[:, f] - (FL[:, f] + th_o * C[:, f])) / scale) < 1e-10, f
+        if linear[f]:
+            assert abs(th_o - theta[f]) < 1e-8, (f, th_o, theta[f])          # exact: on the boundary g = delta
+        else:
+            assert -1e-9 <= th_o <= theta[f] + 1e-8 and admissible(f, max(th_o, 0.0), slack=1e-9), (f, th_o, theta[f])
+    o.close()

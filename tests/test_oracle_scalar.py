@@ -190,6 +190,21 @@ def test_p3_nonlinear_weights_limits(oracle):
     assert om[3] > 1 - 1e-6 and abs(oracle.weno7(v) - 5.0) < 1e-5
 
 
+def test_p3_weight_exponent_and_epsilon_R3(oracle):
+    """Reading R3 (WENO-JS: omega_k ~ d_k / (eps + beta_k)^2, eps absolute): the weight RATIOS follow from the smoothness
+    indicators of the integral definition (computed here by quadrature of the sub-stencil cubics, not by the oracle).
+    An exponent of 1, or an eps that scales with the data, fails this."""
+    rng = np.random.default_rng(19)
+    for scale in (1e-3, 1.0, 50.0):
+        v = scale * rng.normal(size=7)
+        for eps in (1e-6, 1e-2):
+            om = oracle.weno7_parts(v, eps)[3]
+            beta = np.array([_beta_from_definition(v[k:k + 4], 3 - k) for k in range(4)])
+            for k in range(1, 4):
+                expect = (D_IDEAL[k] / D_IDEAL[0]) * ((eps + beta[0]) / (eps + beta[k])) ** 2
+                assert abs(om[k] / om[0] - expect) < 1e-9 * expect, (scale, eps, k)
+
+
 def _fd_derivative_error(oracle, f, dfdx, n, eps):
     """(W_{i+1/2} - W_{i-1/2})/dx vs f'(x_i) with point values f(x_i): the finite-difference use of O5-O7."""
     dx = 1.0 / n
