@@ -45,9 +45,26 @@ FLOPS_SWEEPS_STAGE = {4: 3 * (1208.0 + 12.0) + 20.0, 5: 3 * (1510.0 + 15.0) + 25
 FLOPS_STAGE_W5 = {4: 1820.0, 5: 2261.0}
 FLOPS_SWEEPS_STAGE_W5 = {4: 3 * (560.0 + 12.0) + 20.0, 5: 3 * (700.0 + 15.0) + 25.0}
 FP64_NOMINAL_TF = 148 * 64 * 2 * 1.965e9 / 1e12          # 148 SMs x 64 DFMA/clk x 2 x 1.965 GHz = 37.2
-# dram__bytes_read.sum + dram__bytes_write.sum per sweep launch at 256^3 fp64 nf=4, mean of the x (COMBINE), y and z
-# (REDUCE) kernels, from the one `ncu --set full` capture summarised in profiles/r1_i_ring_ncu_summary.txt
-NCU_TRAFFIC_SWEEP_256_F64_NF4 = (1.315e9 + 1.839e9 + 1.841e9) / 3.0
+# Counters that only ncu can give (DRAM bytes, FP64 warp instructions, pipe utilisation, registers, occupancy) are READ from
+# the committed summary of the `ncu --set full` captures, never typed in here; every row carries the sha of the CUDA
+# sources it was taken at (paper_1511_02137_b200.build.source_sha) and the bench line says when that differs from HEAD.
+NCU_TABLE = os.path.join(ROOT, "profiles", "r2_ncu_kernels.csv")
+
+
+def variant_key(cfg, precision, order, nf, limiter):
+    return "cfg%d_f%d_w%d_nf%d_lim%d" % (cfg, precision, order, nf, 1 if limiter else 0)
+
+
+def ncu_rows(variant):
+    """{kernel class: row dict} of the committed ncu summary for this variant ({} if none)."""
+    import csv
+    out = {}
+    if os.path.exists(NCU_TABLE):
+        with open(NCU_TABLE) as f:
+            for row in csv.DictReader(l for l in f if not l.startswith("#")):
+                if row["variant"] == variant:
+                    out[row["kernel"]] = row
+    return out
 
 
 def max_over_ranks(values, world, device):
@@ -191,8 +208,8 @@ def run_decomposed(args, rank, world, local, barrier):
                  weno_order=args.weno_order)
     for pos, d in c["jets"]:
         sl.g.add_jet(pos, d, S.KAPPA_RAD, S.KAPPA_COLL, S.CR_OVER_CF)
-    sl.g.set_deposit_width(args.deposit_sigma)
-    sl.g.set_limiter(args.limiter)
+    sl.set_deposit_width(args.deposit_sigma)
+    sl.set_limiter(args.limiter)
     d_ = dist if world > 1 else None
     sl.set_state(U0)
     SL.run_distributed(sl, args.warmup, d_)
@@ -291,7 +308,8 @@ def main():
     # ---- measured ALU peak of this GPU, same run
     peak_tf = H.measure_alu_peak(args.precision, 200.0, stream.cuda_stream)
 
-    # ---- warm-up, then the device-resident timed region: K steps from the initial state
+    # ---- warm-up, then the device-resident timed region: K steps from the initial state, as a user runs them (hydro_step
+    # replays one captured RK3 step as a CUDA graph; profiling off)
     g.set_state(U0d)
     g.step(args.warmup)
     g.set_state(U0d)
@@ -300,7 +318,6 @@ def main():
                            os.environ["CUDA_VISIBLE_DEVICES"].split(",")[local])
     sampler.start()
     time.sleep(0.3)
-    g.set_profiling(True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     n0 = g.launch_count()
     barrier()
@@ -313,12 +330,23 @@ def main():
     w1 = time.perf_counter()
     ms = e0.elapsed_time(e1)
     launches = g.launch_count() - n0
-    kt = g.kernel_times()
-    g.set_profiling(False)
     clocks = sampler.stop(w0, w1)
     dg = g.diag()
     if dg["has_nan"]:
         raise SystemExit("bench.py: non-finite state after the timed run")
+    # ---- the same K steps again with one CUDA event after every launch (hydro_set_profiling): per-kernel-class device
+    # times for the roofline of the dominant kernel; individual launches, so this pass is not the reported value
+    g.set_state(U0d)
+    g.synchronize()
+    g.set_profiling(True)
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(stream):
+        p0.record(stream)
+        g.step(args.steps)
+        p1.record(stream)
+    kt = g.kernel_times()
+    g.set_profiling(False)
+    ms_profiled = p0.elapsed_time(p1)
 
     # ---- end to end through the C ABI with HOST buffers: upload, K steps, download, all inside the timed region
     e2e = None
@@ -348,6 +376,20 @@ def main():
         fl_launch = fl_sweeps / 3.0 * cells
         achieved = fl_launch / (sw_ms / sw_n * 1e-3) / 1e12 if sw_n else 0.0
         nominal = FP64_NOMINAL_TF * (1 if args.precision == 64 else 2)
+        esz = args.precision // 8
+        sweeps_per_step = sw_n / args.steps if sw_n else 9.0
+        rows = ncu_rows(variant_key(cfg, args.precision, args.weno_order, nf, args.limiter))
+        from paper_1511_02137_b200 import build as B
+        sha = B.source_sha()
+        srows = [rows[k] for k in ("sweep_x", "sweep_y", "sweep_z") if k in rows]
+        traffic = inst64 = pipe = None
+        if srows:
+            # per launch, mean over the step's sweep launches: stage 1's x kernel (COMBINE1) reads no U^n and is listed
+            # separately when it was captured
+            traffic = sum(float(r["dram_read_B"]) + float(r["dram_write_B"]) for r in srows) / len(srows)
+            inst64 = sum(float(r["inst_fp64"]) for r in srows) / len(srows)
+            pipe = sum(float(r["pipe_fp64_pct"]) for r in srows) / len(srows) / 100.0
+        avg_s = sw_ms / sw_n * 1e-3 if sw_n else None
         roof = {"bound": "alu", "kernel": "k_sweep_ring<x|y|z> (WENO%d-LF flux + divergence + RK3 combine)" % args.weno_order,
                 "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf,
                 "peak_kind": "measured in this run: register-resident %s chain on all SMs (hydro_measure_alu_peak)" %
@@ -356,11 +398,24 @@ def main():
                 "flops_per_launch": fl_launch, "avg_launch_ms": sw_ms / sw_n if sw_n else None,
                 "share_of_step": sw_ms / all_ms if all_ms else None,
                 "kernel_ms_per_step": {k: v["ms"] / args.steps for k, v in kt.items()},
+                "ms_per_step_profiled_pass": ms_profiled / args.steps,
                 "whole_path_frac": (fl_stage * 3 * value) / (peak_tf * 1e12),
-                "fp64_pipe_busy_ncu": 0.856 if (cfg == 3 and args.precision == 64 and args.weno_order == 7 and not args.limiter) else None,
-                "traffic": NCU_TRAFFIC_SWEEP_256_F64_NF4 if (cfg == 3 and args.precision == 64 and args.weno_order == 7) else None,
-                "traffic_source": "profiles/r1_i_ring_ncu_summary.txt (ncu --set full, dram read+write per launch)",
-                "algorithmic_bytes_per_launch": (nf + 2 + nf + nf * 2.0 / 9.0 + 2.0 / 3.0 * nf) * 8.0 * cells}
+                # instruction-level fraction: FP64 warp instructions (ncu) x 32 lanes x 2 flops, as if every one were an
+                # FMA, over the live launch time and the measured FMA peak: cannot exceed 1, unlike the textbook `frac`
+                "inst_frac": (inst64 * 64.0 / avg_s / 1e12 / peak_tf) if (inst64 and avg_s and args.precision == 64) else None,
+                "fp64_warp_inst_per_launch_ncu": inst64,
+                "fp64_pipe_busy_ncu": pipe if args.precision == 64 else None,
+                "traffic": traffic,
+                "traffic_source": "profiles/r2_ncu_kernels.csv (ncu --set full: dram__bytes_read.sum + dram__bytes_write.sum per "
+                                  "launch, mean of the x, y, z sweep kernels)" if srows else None,
+                "profile_csrc_sha": srows[0]["csrc_sha"] if srows else None, "csrc_sha": sha,
+                "profile_stale": (srows[0]["csrc_sha"] != sha) if srows else None,
+                # unique bytes of a fully fused stage, (2 + 3 + 3) x nf x sizeof(real) per cell-update, spread
+                # over the step's sweep launches; traffic / this = how far the three-pass design is from that floor
+                "algorithmic_bytes_per_launch": 8.0 * nf * esz * cells / sweeps_per_step,
+                # what THIS design's sweep kernels must move per launch (U, W, P read; nf written or reduce-added; U^n
+                # read by the COMBINE kernels of stages 2 and 3), mean over the step's launches
+                "kernel_bytes_per_launch": (nf + 2 + nf + nf * 2.0 / 9.0 + 2.0 / 3.0 * nf) * esz * cells}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,

@@ -87,19 +87,37 @@ int hydro_set_step(hydro_t *h, long long step);
  * grid, k_offset = global index of local plane 0, [own_lo, own_hi) = owned local planes (>= 4 of them; an interior end
  * needs its 4 halo planes: HYDRO_EINVAL otherwise).  Jet positions stay global; cap events and jet bookkeeping are
  * counted for owned planes only, so sums over ranks are the global figures.
- * One RK3 step = for s in 0, 1, 2:
+ * One RK3 step = for s in 0, 1, 2 (serial form):
  *     hydro_stage_prims(h, s)                      con2prim + LOCAL wavespeed maxima of stage s's input state
  *     hydro_stage_alpha(h, s, 0, a); a = MAX over ranks; hydro_stage_alpha(h, s, 1, a)      (host round trip, 24 bytes)
+ *       or, without leaving the device: hydro_stage_alpha_dev(h, s, 0, bits); MAX all-reduce of the three 64-bit
+ *       integers (non-negative reals order like their bit patterns); hydro_stage_alpha_dev(h, s, 1, bits)
  *     hydro_stage_sweeps(h, s)                     sweeps + source + stage combination -> stage s's output state
  *     hydro_halo(h, s, side, 0, buf)  pack the 4 owned boundary planes (side 0: low z, 1: high z) of that output state,
  *                                     all fields, into the DEVICE buffer buf (nfields * 4 * ny * pitch reals, see
  *                                     hydro_halo_reals); exchange with the neighbour; hydro_halo(h, s, side, 1, buf) unpacks
  *                                     the neighbour's planes into the halo.  Asynchronous on the handle's stream.
- * hydro_stage_sweeps(h, 2) advances the step counter.  Owned planes come out bitwise identical to the one-GPU run. */
+ * Overlapped form (the halos of stage s's INPUT state may still be in flight; not with the limiter or a Gaussian deposit,
+ * which need the halos before the x sweep: HYDRO_ESTATE):
+ *     hydro_stage_prims_part(h, s, 0)              owned planes: con2prim + local wavespeed maxima
+ *     alpha exchange as above
+ *     hydro_stage_sweeps_part(h, s, 0)             x sweep + source + y sweep on the owned planes (no z neighbour needed)
+ *     wait for the halos of the input state, hydro_halo(..., unpack)
+ *     hydro_stage_prims_part(h, s, 1)              halo planes: con2prim only
+ *     hydro_stage_sweeps_part(h, s, 1)             z sweep (marches the whole local array)
+ *     pack and send the boundary planes of the output state
+ * hydro_stage_sweeps(h, 2) / hydro_stage_sweeps_part(h, 2, 1) advance the step counter.  Owned planes come out bitwise
+ * identical to the one-GPU run in both forms.  With a Gaussian deposit (hydro_set_deposit_width) the cube's half-width
+ * R must not exceed the 4 halo planes (sigma <= 4 dx / 3): HYDRO_EINVAL otherwise. */
 int hydro_set_slab(hydro_t *h, int nz_global, int k_offset, int own_lo, int own_hi);
 int hydro_stage_prims(hydro_t *h, int s);
 int hydro_stage_alpha(hydro_t *h, int s, int set, double alpha[3]);
 int hydro_stage_sweeps(hydro_t *h, int s);
+int hydro_stage_prims_part(hydro_t *h, int s, int part);
+int hydro_stage_sweeps_part(hydro_t *h, int s, int part);
+/* dev_bits: DEVICE pointer to three 64-bit integers.  set = 0: copy the stage's three alpha bit patterns out; 1: in.
+ * Asynchronous on the handle's stream; no host synchronisation. */
+int hydro_stage_alpha_dev(hydro_t *h, int s, int set, void *dev_bits);
 int hydro_halo(hydro_t *h, int s, int side, int unpack, void *dev_buf);
 long long hydro_halo_reals(const hydro_t *h);
 

@@ -41,11 +41,21 @@ struct hydro {
     long long step;
     int prim_slot;                      // DiagSlot holding alpha of buf[cur]'s primitives
     bool prims_valid;
-    // ring sweeps (fp64, even nx): tensor maps per buffer and direction, march cells per block
-    CUtensorMap mapU[3][3], mapW[3], mapP[3], mapL[3];
+    // ring sweeps: tensor maps per buffer (0..2 state copies, 3 = L) and direction, march cells per block
+    CUtensorMap mapB[4][3], mapW[3], mapP[3];
+    // z-slab decomposition: the same maps over the OWNED planes only (x/y sweeps of the owned planes while the halos are
+    // still in flight; output clipping of the z sweep); built by hydro_set_slab
+    CUtensorMap vmapB[4][3], vmapW[3], vmapP[3];
+    bool view;                          // launch the sweeps on the owned-planes view (hydro_stage_sweeps_part)
     int seg_len[3], tma_nseg[3];
     int num_sms;
     long long launches;
+    // one RK3 step captured as a CUDA graph (replayed by hydro_step when profiling is off): valid for graph_slot only and
+    // until the jets, the limiter, the deposit width or the slab change
+    cudaGraphExec_t graph;
+    int graph_slot, graph_njets;
+    long long graph_launches;           // kernel launches inside the graph
+    bool use_graph;                     // HYDRO_NO_GRAPH=1 disables
     // profiling
     bool profiling;
     std::vector<EvSpan> ev_inflight;
@@ -116,14 +126,18 @@ void drain_events(hydro* h) {
     h->chain_prev = 0;
 }
 
+// con2prim (+ wavespeed maxima if with_alpha) of the z planes [k0, k1); reset: clear the DiagSlot first
 template <typename R>
-int launch_prim(hydro* h, const void* U, int slot) {
-    CK(cudaMemsetAsync(&h->diag->slot[slot], 0, sizeof(DiagSlot), h->stream));
+int launch_prim_range(hydro* h, const void* U, int slot, int k0, int k1, bool reset, bool with_alpha) {
+    if (reset) CK(cudaMemsetAsync(&h->diag->slot[slot], 0, sizeof(DiagSlot), h->stream));
+    if (k1 <= k0) return HYDRO_OK;
+    const long long plane = (long long)h->nx * h->ny;
     PrimArgs<R> a;
-    a.U = (const R*)U; a.P = (R*)h->P; a.W = (R*)h->W; a.diag = h->diag; a.slot = slot; a.N = h->N; a.Np = h->Np; a.nx = h->nx; a.nxp = h->nxp;
-    a.own_lo = (long long)h->own_lo * h->nx * h->ny; a.own_hi = (long long)h->own_hi * h->nx * h->ny;
+    a.U = (const R*)U; a.P = (R*)h->P; a.W = (R*)h->W; a.diag = h->diag; a.slot = slot; a.c0 = k0 * plane; a.N = k1 * plane;
+    a.Np = h->Np; a.nx = h->nx; a.nxp = h->nxp; a.with_alpha = with_alpha ? 1 : 0;
+    a.own_lo = (long long)h->own_lo * plane; a.own_hi = (long long)h->own_hi * plane;
     a.e_floor = (R)h->e_floor; a.one_minus_delta = (R)(1.0 - h->delta);
-    long long blocks = (h->N + 255) / 256;
+    long long blocks = (a.N - a.c0 + 255) / 256;
     long long cap = (long long)h->num_sms * 8;
     if (blocks > cap) blocks = cap;
     {
@@ -134,31 +148,43 @@ int launch_prim(hydro* h, const void* U, int slot) {
     CK(cudaGetLastError());
     return HYDRO_OK;
 }
+template <typename R>
+int launch_prim(hydro* h, const void* U, int slot) { return launch_prim_range<R>(h, U, slot, 0, h->nz, true, true); }
 
+// 0..2: the state copies, 3: the RHS buffer L
 int buf_index(const hydro* h, const void* U) {
     for (int b = 0; b < 3; ++b) if (h->buf[b] == U) return b;
-    return -1;
+    return U == h->L ? 3 : -1;
 }
 
-// One ring sweep (hydro_sweep_ring.cuh).  `Us` must be one of the three state buffers; `out_map` is the tensor map
-// (for direction DIR) of the buffer the result is stored / reduced into; `un_map` that of U^n (OUT_COMBINE).
+// One ring sweep (hydro_sweep_ring.cuh).  `Us` must be one of the three state buffers; `out_b` is the buffer (0..2 state
+// copy, 3 = L) the result is stored / reduced into; `un_b` that of U^n (OUT_COMBINE; < 0: none).
 // LIM = 1 (fp64 only): the limited scheme of R16, U^L is read from h->L.
+// h->view (z-slabs): the x and y sweeps run on the owned planes only (all maps are the owned-planes views, the kernel
+// sees a grid of own_hi - own_lo planes); the z sweep marches the whole local array as always (what it adds to the halo
+// planes of the target is overwritten by the next exchange).
 template <typename R, int ORDER, int LIM, int DIR, int OUT, int NF>
-int launch_ring_nf(hydro* h, const void* Us, int slot, const CUtensorMap* out_map, const CUtensorMap* un_map, double coef,
-                   double rk_a, double rk_b) {
+int launch_ring_nf(hydro* h, const void* Us, int slot, int out_b, int un_b, double coef, double rk_a, double rk_b) {
     if constexpr (LIM && sizeof(R) != 8) return HYDRO_ESTATE;
     else {
         const int b = buf_index(h, Us);
-        if (b < 0) return HYDRO_ESTATE;
+        if (b < 0 || b > 2 || out_b < 0 || out_b > 3 || un_b > 2) return HYDRO_ESTATE;
+        const bool vw = h->view && DIR != 2;                               // everything through the owned-planes view
         RingMaps m;
-        m.U = h->mapU[b][DIR]; m.W = h->mapW[DIR]; m.P = h->mapP[DIR]; m.Out = *out_map; m.Un = un_map ? *un_map : *out_map;
-        m.UL = h->mapL[DIR];
+        m.U = vw ? h->vmapB[b][DIR] : h->mapB[b][DIR];
+        m.W = vw ? h->vmapW[DIR] : h->mapW[DIR];
+        m.P = vw ? h->vmapP[DIR] : h->mapP[DIR];
+        m.Out = vw ? h->vmapB[out_b][DIR] : h->mapB[out_b][DIR];
+        m.Un = un_b >= 0 ? (vw ? h->vmapB[un_b][DIR] : h->mapB[un_b][DIR]) : m.Out;
+        m.UL = vw ? h->vmapB[3][DIR] : h->mapB[3][DIR];
+        const int nz_k = vw ? h->own_hi - h->own_lo : h->nz;              // planes the kernel sees
         RingArgs a;
-        a.diag = h->diag; a.slot = slot; a.nx = h->nx; a.ny = h->ny; a.nz = h->nz; a.seg_len = h->seg_len[DIR];
+        a.diag = h->diag; a.slot = slot; a.nx = h->nx; a.ny = h->ny; a.nz = nz_k; a.seg_len = h->seg_len[DIR];
         a.eps_eff = (ORDER == 5 ? 48.0 : 144.0) * h->weno_eps; a.coef = coef; a.dt = h->dt; a.rk_a = rk_a; a.rk_b = rk_b;
         a.k3lam = 3.0 * h->dt / h->dx; a.nlim = &h->diag->nlim_total;
+        a.own_lo = vw ? 0 : h->own_lo; a.own_hi = vw ? nz_k : h->own_hi;
         const int nlane = DIR == 0 ? h->ny : h->nx;
-        const int other = DIR == 2 ? h->ny : h->nz;
+        const int other = DIR == 2 ? h->ny : nz_k;
         const int nd = DIR == 0 ? h->nx : DIR == 1 ? h->ny : h->nz;
         const long long tiles = (long long)((nlane + 31) / 32) * other;
         dim3 grid((unsigned)tiles, (unsigned)h->tma_nseg[DIR], 1);
@@ -193,19 +219,17 @@ int launch_ring_nf(hydro* h, const void* Us, int slot, const CUtensorMap* out_ma
 }
 
 template <typename R, int LIM, int DIR, int OUT>
-int launch_ring_lim(hydro* h, const void* Us, int slot, const CUtensorMap* out_map, const CUtensorMap* un_map, double coef,
-                    double rk_a, double rk_b) {
+int launch_ring_lim(hydro* h, const void* Us, int slot, int out_b, int un_b, double coef, double rk_a, double rk_b) {
     if (h->order == 5)
-        return h->nf == 4 ? launch_ring_nf<R, 5, LIM, DIR, OUT, 4>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b)
-                          : launch_ring_nf<R, 5, LIM, DIR, OUT, 5>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b);
-    return h->nf == 4 ? launch_ring_nf<R, 7, LIM, DIR, OUT, 4>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b)
-                      : launch_ring_nf<R, 7, LIM, DIR, OUT, 5>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b);
+        return h->nf == 4 ? launch_ring_nf<R, 5, LIM, DIR, OUT, 4>(h, Us, slot, out_b, un_b, coef, rk_a, rk_b)
+                          : launch_ring_nf<R, 5, LIM, DIR, OUT, 5>(h, Us, slot, out_b, un_b, coef, rk_a, rk_b);
+    return h->nf == 4 ? launch_ring_nf<R, 7, LIM, DIR, OUT, 4>(h, Us, slot, out_b, un_b, coef, rk_a, rk_b)
+                      : launch_ring_nf<R, 7, LIM, DIR, OUT, 5>(h, Us, slot, out_b, un_b, coef, rk_a, rk_b);
 }
 template <typename R, int DIR, int OUT>
-int launch_ring(hydro* h, const void* Us, int slot, const CUtensorMap* out_map, const CUtensorMap* un_map, double coef,
-                double rk_a, double rk_b) {
-    return h->limiter ? launch_ring_lim<R, 1, DIR, OUT>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b)
-                      : launch_ring_lim<R, 0, DIR, OUT>(h, Us, slot, out_map, un_map, coef, rk_a, rk_b);
+int launch_ring(hydro* h, const void* Us, int slot, int out_b, int un_b, double coef, double rk_a, double rk_b) {
+    return h->limiter ? launch_ring_lim<R, 1, DIR, OUT>(h, Us, slot, out_b, un_b, coef, rk_a, rk_b)
+                      : launch_ring_lim<R, 0, DIR, OUT>(h, Us, slot, out_b, un_b, coef, rk_a, rk_b);
 }
 
 template <typename R, int LIM, int DIR, int OUT, int NF>
@@ -226,8 +250,9 @@ int set_smem_attrs() {
            set_smem_attr<R, 1, 2, OUT_REDUCE, NF>();
 }
 
-// 4-D tensor map (x, y, z, field) of one SoA buffer with `nfb` fields; box given per dimension
-int make_map(hydro* h, CUtensorMap* out, void* base, int nfb, const unsigned box[4], bool swizzle64) {
+// 4-D tensor map (x, y, z, field) of the z planes [k0, k1) of one SoA buffer with `nfb` fields; box given per dimension
+int make_map(hydro* h, CUtensorMap* out, void* base0, int nfb, const unsigned box[4], bool swizzle64, int k0, int k1) {
+    void* base = (char*)base0 + (size_t)k0 * h->nxp * h->ny * h->esz;
     static PFN_cuTensorMapEncodeTiled_v12000 encode = 0;
     if (!encode) {
         void* fn = 0;
@@ -239,7 +264,7 @@ int make_map(hydro* h, CUtensorMap* out, void* base, int nfb, const unsigned box
         }
         encode = (PFN_cuTensorMapEncodeTiled_v12000)fn;
     }
-    cuuint64_t gdim[4] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny, (cuuint64_t)h->nz, (cuuint64_t)nfb};
+    cuuint64_t gdim[4] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny, (cuuint64_t)(k1 - k0), (cuuint64_t)nfb};
     const cuuint64_t es8 = (cuuint64_t)h->esz;
     cuuint64_t gstr[3] = {(cuuint64_t)h->nxp * es8, (cuuint64_t)h->nxp * h->ny * es8, (cuuint64_t)h->Np * es8};
     cuuint32_t bx[4] = {box[0], box[1], box[2], box[3]};
@@ -259,18 +284,25 @@ int make_map(hydro* h, CUtensorMap* out, void* base, int nfb, const unsigned box
     return HYDRO_OK;
 }
 
-int setup_tma(hydro* h) {
+// tensor maps of the planes [k0, k1) of every buffer, per direction
+int build_maps(hydro* h, CUtensorMap mB[4][3], CUtensorMap mW[3], CUtensorMap mP[3], int k0, int k1) {
     const unsigned NF = (unsigned)h->nf;
     const unsigned boxes[3][4] = {{RING_CH, 32, 1, NF}, {32, RING_CH, 1, NF}, {32, 1, RING_CH, NF}};
     int rc;
     for (int d = 0; d < 3; ++d) {
         unsigned b1[4] = {boxes[d][0], boxes[d][1], boxes[d][2], 1};
-        for (int b = 0; b < 3; ++b)
-            if ((rc = make_map(h, &h->mapU[b][d], h->buf[b], h->nf, boxes[d], d == 0)) != HYDRO_OK) return rc;
-        if ((rc = make_map(h, &h->mapW[d], h->W, 1, b1, d == 0)) != HYDRO_OK) return rc;
-        if ((rc = make_map(h, &h->mapP[d], h->P, 1, b1, d == 0)) != HYDRO_OK) return rc;
-        if ((rc = make_map(h, &h->mapL[d], h->L, h->nf, boxes[d], d == 0)) != HYDRO_OK) return rc;
+        for (int b = 0; b < 4; ++b)
+            if ((rc = make_map(h, &mB[b][d], b < 3 ? h->buf[b] : h->L, h->nf, boxes[d], d == 0, k0, k1)) != HYDRO_OK) return rc;
+        if ((rc = make_map(h, &mW[d], h->W, 1, b1, d == 0, k0, k1)) != HYDRO_OK) return rc;
+        if ((rc = make_map(h, &mP[d], h->P, 1, b1, d == 0, k0, k1)) != HYDRO_OK) return rc;
     }
+    return HYDRO_OK;
+}
+
+int setup_tma(hydro* h) {
+    int rc;
+    if ((rc = build_maps(h, h->mapB, h->mapW, h->mapP, 0, h->nz)) != HYDRO_OK) return rc;
+    if ((rc = build_maps(h, h->vmapB, h->vmapW, h->vmapP, 0, h->nz)) != HYDRO_OK) return rc;
     const int bad = h->prec == 64 ? (h->nf == 4 ? set_smem_attrs<double, 4>() : set_smem_attrs<double, 5>())
                                   : (h->nf == 4 ? set_smem_attrs<float, 4>() : set_smem_attrs<float, 5>());
     if (bad) {
@@ -307,12 +339,15 @@ int upload_jets(hydro* h) {
 }
 
 template <typename R>
-int launch_source(hydro* h, int slot, int stage, double stage_c, bool commit, double rk_weight, void* target, double scale) {
+int launch_source(hydro* h, int slot, int stage, double stage_c, bool commit, double rk_weight, void* target, double scale,
+                  bool advance = false) {
     int rc;
     if ((rc = upload_jets<R>(h)) != HYDRO_OK) return rc;
     SourceArgs s;
     s.diag = h->diag; s.jets = h->jets_dev; s.njets = (int)h->jets.size(); s.slot = slot; s.stage = stage;
-    s.commit = commit ? 1 : 0; s.nx = h->nx; s.ny = h->ny; s.nz = h->nz; s.nxp = h->nxp; s.N = h->Np; s.step = h->step;
+    s.commit = commit ? 1 : 0; s.nx = h->nx; s.ny = h->ny; s.nz = h->nz; s.nxp = h->nxp; s.N = h->Np;
+    s.zero_slot = commit ? (slot + 1) % NSLOT : -1;                 // the slot the next k_prim fills
+    s.advance = advance ? 1 : 0;
     s.nz_global = h->nz_global; s.k_offset = h->k_offset; s.own_lo = h->own_lo; s.own_hi = h->own_hi;
     s.stage_c = stage_c; s.dx = h->dx; s.dt = h->dt; s.rk_weight = rk_weight; s.scale = scale; s.sigma = h->sigma;
     {
@@ -324,14 +359,17 @@ int launch_source(hydro* h, int slot, int stage, double stage_c, bool commit, do
     return HYDRO_OK;
 }
 
-// Ring path (fp64, even nx).  With Uout: the x sweep stores U_next = a U^n + b (U_s + dt L_x), the source kernel and
-// the y, z sweeps add b dt S, b dt L_y, b dt L_z to it (the stage update is linear in L).  Without: L into h->L.
+// With Uout: the x sweep stores U_next = a U^n + b (U_s + dt L_x), the source kernel and the y, z sweeps add b dt S,
+// b dt L_y, b dt L_z to it (the stage update is linear in L).  Without: L into h->L.
+// `parts`: bit 0 = x sweep + source + y sweep, bit 1 = z sweep (3 = the whole stage; the split serves the z-slab overlap:
+// x and y need no z halos).  The limiter path and hydro_eval_rhs always run whole.
 template <typename R>
 int eval_stage_ring(hydro* h, const void* Uin, int slot, int stage, double stage_c, bool commit, double rk_weight,
-                    void* Uout, const void* Un, double rk_a, double rk_b) {
+                    void* Uout, const void* Un, double rk_a, double rk_b, int parts = 3) {
     const double hid = 0.5 / h->dx;
     int rc;
     if (h->limiter) {
+        if (parts != 3) return HYDRO_ESTATE;
         // R16: U^L (first-order update) into h->L, then the sweeps add only theta x (WENO correction) to it
         LowArgs<R> la;
         la.U = (const R*)Uin; la.P = (const R*)h->P; la.W = (const R*)h->W; la.UL = (R*)h->L; la.diag = h->diag; la.slot = slot;
@@ -355,40 +393,48 @@ int eval_stage_ring(hydro* h, const void* Uin, int slot, int stage, double stage
             void* Ue = h->buf[(h->cur + 1) % 3];
             void* Ld = h->buf[(h->cur + 2) % 3];
             const int be = buf_index(h, Ue);
-            if ((rc = launch_ring<R, 0, OUT_COMBINE1>(h, Uin, slot, &h->mapU[be][0], 0, hid, 0.0, 1.0)) != HYDRO_OK) return rc;
+            if ((rc = launch_ring<R, 0, OUT_COMBINE1>(h, Uin, slot, be, -1, hid, 0.0, 1.0)) != HYDRO_OK) return rc;
             if ((rc = launch_source<R>(h, slot, stage, stage_c, commit, rk_weight, Ue, h->dt)) != HYDRO_OK) return rc;
-            if ((rc = launch_ring<R, 1, OUT_REDUCE>(h, Uin, slot, &h->mapU[be][1], 0, h->dt * hid, 0.0, 0.0)) != HYDRO_OK) return rc;
-            if ((rc = launch_ring<R, 2, OUT_REDUCE>(h, Uin, slot, &h->mapU[be][2], 0, h->dt * hid, 0.0, 0.0)) != HYDRO_OK) return rc;
+            if ((rc = launch_ring<R, 1, OUT_REDUCE>(h, Uin, slot, be, -1, h->dt * hid, 0.0, 0.0)) != HYDRO_OK) return rc;
+            if ((rc = launch_ring<R, 2, OUT_REDUCE>(h, Uin, slot, be, -1, h->dt * hid, 0.0, 0.0)) != HYDRO_OK) return rc;
             const long long n = h->Np * h->nf;
             long long bl = (n + 255) / 256;
             if (bl > (long long)h->num_sms * 16) bl = (long long)h->num_sms * 16;
-            k_diff<R><<<(unsigned)bl, 256, 0, h->stream>>>((const R*)Ue, (const R*)Uin, (R*)Ld, n, (R)(1.0 / h->dt));
+            {
+                Timer t(h, HYDRO_K_PRIM);
+                k_diff<R><<<(unsigned)bl, 256, 0, h->stream>>>((const R*)Ue, (const R*)Uin, (R*)Ld, n, (R)(1.0 / h->dt));
+            }
+            h->launches += 1;
             CK(cudaGetLastError());
             return HYDRO_OK;
         }
     }
     if (Uout) {
         const int bo = buf_index(h, Uout), bn = Un ? buf_index(h, Un) : -1;
-        if (bo < 0 || (Un && bn < 0)) return HYDRO_ESTATE;
-        if (Un) rc = launch_ring<R, 0, OUT_COMBINE>(h, Uin, slot, &h->mapU[bo][0], &h->mapU[bn][0], hid, rk_a, rk_b);
-        else rc = launch_ring<R, 0, OUT_COMBINE1>(h, Uin, slot, &h->mapU[bo][0], 0, hid, 0.0, 1.0);
-        if (rc != HYDRO_OK) return rc;
+        if (bo < 0 || bo > 2 || (Un && (bn < 0 || bn > 2))) return HYDRO_ESTATE;
         const double bdt = (Un ? rk_b : 1.0) * h->dt;
-        if ((rc = launch_source<R>(h, slot, stage, stage_c, commit, rk_weight, Uout, bdt)) != HYDRO_OK) return rc;
-        if ((rc = launch_ring<R, 1, OUT_REDUCE>(h, Uin, slot, &h->mapU[bo][1], 0, bdt * hid, 0.0, 0.0)) != HYDRO_OK) return rc;
-        return launch_ring<R, 2, OUT_REDUCE>(h, Uin, slot, &h->mapU[bo][2], 0, bdt * hid, 0.0, 0.0);
+        if (parts & 1) {
+            if (Un) rc = launch_ring<R, 0, OUT_COMBINE>(h, Uin, slot, bo, bn, hid, rk_a, rk_b);
+            else rc = launch_ring<R, 0, OUT_COMBINE1>(h, Uin, slot, bo, -1, hid, 0.0, 1.0);
+            if (rc != HYDRO_OK) return rc;
+            if ((rc = launch_source<R>(h, slot, stage, stage_c, commit, rk_weight, Uout, bdt, commit && stage == 2)) != HYDRO_OK) return rc;
+            if ((rc = launch_ring<R, 1, OUT_REDUCE>(h, Uin, slot, bo, -1, bdt * hid, 0.0, 0.0)) != HYDRO_OK) return rc;
+        }
+        if (parts & 2) return launch_ring<R, 2, OUT_REDUCE>(h, Uin, slot, bo, -1, bdt * hid, 0.0, 0.0);
+        return HYDRO_OK;
     }
-    if ((rc = launch_ring<R, 0, OUT_STORE>(h, Uin, slot, &h->mapL[0], 0, hid, 0.0, 0.0)) != HYDRO_OK) return rc;
+    if (parts != 3) return HYDRO_ESTATE;
+    if ((rc = launch_ring<R, 0, OUT_STORE>(h, Uin, slot, 3, -1, hid, 0.0, 0.0)) != HYDRO_OK) return rc;
     if ((rc = launch_source<R>(h, slot, stage, stage_c, commit, rk_weight, h->L, 1.0)) != HYDRO_OK) return rc;
-    if ((rc = launch_ring<R, 1, OUT_REDUCE>(h, Uin, slot, &h->mapL[1], 0, hid, 0.0, 0.0)) != HYDRO_OK) return rc;
-    return launch_ring<R, 2, OUT_REDUCE>(h, Uin, slot, &h->mapL[2], 0, hid, 0.0, 0.0);
+    if ((rc = launch_ring<R, 1, OUT_REDUCE>(h, Uin, slot, 3, -1, hid, 0.0, 0.0)) != HYDRO_OK) return rc;
+    return launch_ring<R, 2, OUT_REDUCE>(h, Uin, slot, 3, -1, hid, 0.0, 0.0);
 }
 
 // L(U_in, t_n + stage_c dt) into h->L; if Uout != 0 the stage combination forms the next stage state instead.
 template <typename R>
 int eval_stage(hydro* h, const void* Uin, int slot, int stage, double stage_c, bool commit, double rk_weight,
-               void* Uout, const void* Un, double rk_a, double rk_b) {
-    return eval_stage_ring<R>(h, Uin, slot, stage, stage_c, commit, rk_weight, Uout, Un, rk_a, rk_b);
+               void* Uout, const void* Un, double rk_a, double rk_b, int parts = 3) {
+    return eval_stage_ring<R>(h, Uin, slot, stage, stage_c, commit, rk_weight, Uout, Un, rk_a, rk_b, parts);
 }
 
 template <typename R>
@@ -399,27 +445,72 @@ int ensure_prims(hydro* h) {
     return rc;
 }
 
+// One RK3 step: 15 kernels.  The DiagSlots rotate slot0 -> slot0+1 -> slot0+2 -> slot0 (mod 3), so every step uses the same
+// sequence; nothing the kernels are passed changes from step to step (the step counter lives in diag->step), which is
+// what lets one captured step be replayed.  k_source clears the slot of the following k_prim (no memset nodes).
+template <typename R>
+int enqueue_step(hydro* h) {
+    int rc;
+    void* Un = h->buf[h->cur];
+    void* Ua = h->buf[(h->cur + 1) % 3];
+    void* Ub = h->buf[(h->cur + 2) % 3];
+    const int s0 = h->prim_slot, s1 = (s0 + 1) % NSLOT, s2 = (s0 + 2) % NSLOT;
+    // stage 1: U1 = Un + dt L(Un, t_n)
+    if ((rc = eval_stage<R>(h, Un, s0, 0, 0.0, true, 1.0 / 6.0, Ua, 0, 0.0, 1.0)) != HYDRO_OK) return rc;
+    if ((rc = launch_prim_range<R>(h, Ua, s1, 0, h->nz, false, true)) != HYDRO_OK) return rc;
+    // stage 2: U2 = 3/4 Un + 1/4 (U1 + dt L(U1, t_n + dt))
+    if ((rc = eval_stage<R>(h, Ua, s1, 1, 1.0, true, 1.0 / 6.0, Ub, Un, 0.75, 0.25)) != HYDRO_OK) return rc;
+    if ((rc = launch_prim_range<R>(h, Ub, s2, 0, h->nz, false, true)) != HYDRO_OK) return rc;
+    // stage 3: U^{n+1} = 1/3 Un + 2/3 (U2 + dt L(U2, t_n + dt/2)), written over Un (each cell reads only its own Un)
+    if ((rc = eval_stage<R>(h, Ub, s2, 2, 0.5, true, 2.0 / 3.0, Un, Un, 1.0 / 3.0, 2.0 / 3.0)) != HYDRO_OK) return rc;
+    return launch_prim_range<R>(h, Un, s0, 0, h->nz, false, true);
+}
+
+void drop_graph(hydro* h) {
+    if (h->graph) cudaGraphExecDestroy(h->graph);
+    h->graph = 0;
+}
+
+template <typename R>
+int capture_step(hydro* h) {
+    int rc;
+    if ((rc = upload_jets<R>(h)) != HYDRO_OK) return rc;            // host -> device copies cannot be captured
+    const long long l0 = h->launches;
+    cudaGraph_t g = 0;
+    CK(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+    rc = enqueue_step<R>(h);
+    cudaError_t e = cudaStreamEndCapture(h->stream, &g);
+    h->graph_launches = h->launches - l0;
+    h->launches = l0;                                               // nothing ran yet
+    if (rc != HYDRO_OK) { if (g) cudaGraphDestroy(g); return rc; }
+    if (e != cudaSuccess) return cuda_fail(h, e, "cudaStreamEndCapture");
+    e = cudaGraphInstantiate(&h->graph, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { h->graph = 0; return cuda_fail(h, e, "cudaGraphInstantiate"); }
+    h->graph_slot = h->prim_slot;
+    h->graph_njets = (int)h->jets.size();
+    return HYDRO_OK;
+}
+
 template <typename R>
 int step_impl(hydro* h, int nsteps) {
     int rc;
+    if (nsteps == 0) return HYDRO_OK;
+    if ((rc = ensure_prims<R>(h)) != HYDRO_OK) return rc;
+    const bool graph = h->use_graph && !h->profiling;              // per-kernel event timing needs individual launches
+    if (graph) {
+        if ((rc = upload_jets<R>(h)) != HYDRO_OK) return rc;       // the jet table itself lives in device memory
+        if (!h->graph || h->graph_njets != (int)h->jets.size() || h->graph_slot != h->prim_slot) {
+            drop_graph(h);
+            if ((rc = capture_step<R>(h)) != HYDRO_OK) return rc;
+        }
+    }
     for (int n = 0; n < nsteps; ++n) {
-        if ((rc = ensure_prims<R>(h)) != HYDRO_OK) return rc;
-        void* Un = h->buf[h->cur];
-        void* Ua = h->buf[(h->cur + 1) % 3];
-        void* Ub = h->buf[(h->cur + 2) % 3];
-        int slot = h->prim_slot;
-        // stage 1: U1 = Un + dt L(Un, t_n)
-        if ((rc = eval_stage<R>(h, Un, slot, 0, 0.0, true, 1.0 / 6.0, Ua, 0, 0.0, 1.0)) != HYDRO_OK) return rc;
-        if ((rc = launch_prim<R>(h, Ua, slot ^ 1)) != HYDRO_OK) return rc;
-        // stage 2: U2 = 3/4 Un + 1/4 (U1 + dt L(U1, t_n + dt))
-        if ((rc = eval_stage<R>(h, Ua, slot ^ 1, 1, 1.0, true, 1.0 / 6.0, Ub, Un, 0.75, 0.25)) != HYDRO_OK) return rc;
-        if ((rc = launch_prim<R>(h, Ub, slot)) != HYDRO_OK) return rc;
-        // stage 3: U^{n+1} = 1/3 Un + 2/3 (U2 + dt L(U2, t_n + dt/2)), written over Un (each cell reads only its own Un)
-        if ((rc = eval_stage<R>(h, Ub, slot, 2, 0.5, true, 2.0 / 3.0, Un, Un, 1.0 / 3.0, 2.0 / 3.0)) != HYDRO_OK)
-            return rc;
+        if (graph) {
+            CK(cudaGraphLaunch(h->graph, h->stream));
+            h->launches += h->graph_launches;
+        } else if ((rc = enqueue_step<R>(h)) != HYDRO_OK) return rc;
         h->step += 1;
-        if ((rc = launch_prim<R>(h, Un, slot ^ 1)) != HYDRO_OK) return rc;
-        h->prim_slot = slot ^ 1;
     }
     return HYDRO_OK;
 }
@@ -433,21 +524,32 @@ StagePlan stage_plan(hydro* h, int s) {
     const int slot = h->prim_slot;
     StagePlan p;
     if (s == 0) { p.in = Un; p.out = Ua; p.un = 0; p.slot = slot; p.c = 0.0; p.w = 1.0 / 6.0; p.a = 0.0; p.b = 1.0; }
-    else if (s == 1) { p.in = Ua; p.out = Ub; p.un = Un; p.slot = slot ^ 1; p.c = 1.0; p.w = 1.0 / 6.0; p.a = 0.75; p.b = 0.25; }
-    else { p.in = Ub; p.out = Un; p.un = Un; p.slot = slot; p.c = 0.5; p.w = 2.0 / 3.0; p.a = 1.0 / 3.0; p.b = 2.0 / 3.0; }
+    else if (s == 1) { p.in = Ua; p.out = Ub; p.un = Un; p.slot = (slot + 1) % NSLOT; p.c = 1.0; p.w = 1.0 / 6.0; p.a = 0.75; p.b = 0.25; }
+    else { p.in = Ub; p.out = Un; p.un = Un; p.slot = (slot + 2) % NSLOT; p.c = 0.5; p.w = 2.0 / 3.0; p.a = 1.0 / 3.0; p.b = 2.0 / 3.0; }
     return p;
 }
+// part: -1 = all planes; 0 = the owned planes (+ the local wavespeed maxima and cap counts); 1 = the halo planes
+// (primitives only), to be called once the neighbours' planes have been unpacked
 template <typename R>
-int stage_prims_impl(hydro* h, int s) {
+int stage_prims_impl(hydro* h, int s, int part) {
     const StagePlan p = stage_plan(h, s);
-    return launch_prim<R>(h, p.in, p.slot);
-}
-template <typename R>
-int stage_sweeps_impl(hydro* h, int s) {
-    const StagePlan p = stage_plan(h, s);
-    int rc = eval_stage<R>(h, p.in, p.slot, s, p.c, true, p.w, p.out, p.un, p.a, p.b);
+    if (part < 0) return launch_prim<R>(h, p.in, p.slot);
+    if (part == 0) return launch_prim_range<R>(h, p.in, p.slot, h->own_lo, h->own_hi, true, true);
+    int rc = launch_prim_range<R>(h, p.in, p.slot, 0, h->own_lo, false, false);
     if (rc != HYDRO_OK) return rc;
-    if (s == 2) { h->step += 1; h->prim_slot ^= 1; h->prims_valid = false; }
+    return launch_prim_range<R>(h, p.in, p.slot, h->own_hi, h->nz, false, false);
+}
+// part: -1 = the whole stage on the whole local array; 0 = x sweep + source + y sweep on the owned planes;
+// 1 = z sweep and, for s = 2, the end-of-step bookkeeping
+template <typename R>
+int stage_sweeps_impl(hydro* h, int s, int part) {
+    const StagePlan p = stage_plan(h, s);
+    if (part >= 0 && (h->limiter || h->sigma > 0.0)) return HYDRO_ESTATE;    // those need the halos before the x sweep
+    h->view = part >= 0;
+    int rc = eval_stage<R>(h, p.in, p.slot, s, p.c, true, p.w, p.out, p.un, p.a, p.b, part < 0 ? 3 : part == 0 ? 1 : 2);
+    h->view = false;
+    if (rc != HYDRO_OK) return rc;
+    if (s == 2 && part != 0) { h->step += 1; h->prims_valid = false; }   // the next stage 0 refills slot prim_slot
     return HYDRO_OK;
 }
 
@@ -520,6 +622,9 @@ int hydro_create(hydro_t** out, int nx, int ny, int nz, double dx, double dt, co
     h->cur = 0; h->L = h->P = h->W = 0; h->diag = 0; h->jets_dev = 0;
     h->jets_dirty = false; h->step = 0; h->prim_slot = 0; h->prims_valid = false; h->launches = 0;
     h->profiling = false;
+    h->view = false;
+    h->graph = 0; h->graph_slot = -1; h->graph_njets = -1; h->graph_launches = 0;
+    { const char* ng = getenv("HYDRO_NO_GRAPH"); h->use_graph = !(ng && ng[0] == '1'); }
     h->chain_prev = 0;
     for (int k = 0; k < HYDRO_K_COUNT; ++k) { h->k_ms[k] = 0; h->k_n[k] = 0; }
     int rc = HYDRO_OK;
@@ -563,6 +668,7 @@ void hydro_destroy(hydro_t* h) {
     if (!h) return;
     if (h->stream || !h->own_stream) cudaStreamSynchronize(h->stream);
     drain_events(h);
+    drop_graph(h);
     for (size_t n = 0; n < h->ev_pool.size(); ++n) cudaEventDestroy(h->ev_pool[n]);
     for (int b = 0; b < 3; ++b) cudaFree(h->buf[b]);
     cudaFree(h->L); cudaFree(h->P); cudaFree(h->W); cudaFree(h->diag); cudaFree(h->jets_dev);
@@ -601,24 +707,54 @@ int hydro_add_jet(hydro_t* h, double x0, double y0, double z0, double dirx, doub
     return HYDRO_OK;
 }
 
+// cells of half-width of the Gaussian deposit cube (R15): ceil(3 sigma/dx - 2^-20) clamped to [1, 8]; 0 for the point deposit
+static int deposit_radius(const hydro* h, double sigma) {
+    if (!(sigma > 0.0)) return 0;
+    int r = (int)std::ceil(3.0 * sigma / h->dx - 1.0 / 1048576.0);
+    return r < 1 ? 1 : (r > 8 ? 8 : r);
+}
+static bool is_slab(const hydro* h) { return h->own_lo > 0 || h->own_hi < h->nz; }
+
 int hydro_set_slab(hydro_t* h, int nz_global, int k_offset, int own_lo, int own_hi) {
     if (!h || nz_global < h->nz || k_offset < 0 || k_offset + h->nz > nz_global || own_lo < 0 || own_hi > h->nz || own_lo >= own_hi)
         return HYDRO_EINVAL;
     // an interior slab end must carry the 4 halo planes the stencil needs
     if ((k_offset > 0 && own_lo < 4) || (k_offset + h->nz < nz_global && h->nz - own_hi < 4)) return HYDRO_EINVAL;
+    // a Gaussian deposit wider than the halo would lose the part of its cube that a rank cannot see
+    if ((own_lo > 0 || own_hi < h->nz) && deposit_radius(h, h->sigma) > 4) return HYDRO_EINVAL;
     h->nz_global = nz_global; h->k_offset = k_offset; h->own_lo = own_lo; h->own_hi = own_hi;
     h->prims_valid = false;
-    return HYDRO_OK;
+    drop_graph(h);
+    return build_maps(h, h->vmapB, h->vmapW, h->vmapP, own_lo, own_hi);
 }
 
 int hydro_stage_prims(hydro_t* h, int s) {
     if (!h || s < 0 || s > 2) return HYDRO_EINVAL;
-    return h->prec == 64 ? stage_prims_impl<double>(h, s) : stage_prims_impl<float>(h, s);
+    return h->prec == 64 ? stage_prims_impl<double>(h, s, -1) : stage_prims_impl<float>(h, s, -1);
 }
 
 int hydro_stage_sweeps(hydro_t* h, int s) {
     if (!h || s < 0 || s > 2) return HYDRO_EINVAL;
-    return h->prec == 64 ? stage_sweeps_impl<double>(h, s) : stage_sweeps_impl<float>(h, s);
+    return h->prec == 64 ? stage_sweeps_impl<double>(h, s, -1) : stage_sweeps_impl<float>(h, s, -1);
+}
+
+int hydro_stage_prims_part(hydro_t* h, int s, int part) {
+    if (!h || s < 0 || s > 2 || (part != 0 && part != 1)) return HYDRO_EINVAL;
+    return h->prec == 64 ? stage_prims_impl<double>(h, s, part) : stage_prims_impl<float>(h, s, part);
+}
+
+int hydro_stage_sweeps_part(hydro_t* h, int s, int part) {
+    if (!h || s < 0 || s > 2 || (part != 0 && part != 1)) return HYDRO_EINVAL;
+    return h->prec == 64 ? stage_sweeps_impl<double>(h, s, part) : stage_sweeps_impl<float>(h, s, part);
+}
+
+int hydro_stage_alpha_dev(hydro_t* h, int s, int set, void* dev_bits) {
+    if (!h || s < 0 || s > 2 || !dev_bits) return HYDRO_EINVAL;
+    const StagePlan p = stage_plan(h, s);
+    unsigned long long* slot_bits = h->diag->slot[p.slot].alpha_bits;
+    if (set) CK(cudaMemcpyAsync(slot_bits, dev_bits, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToDevice, h->stream));
+    else CK(cudaMemcpyAsync(dev_bits, slot_bits, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToDevice, h->stream));
+    return HYDRO_OK;
 }
 
 int hydro_stage_alpha(hydro_t* h, int s, int set, double alpha[3]) {
@@ -665,6 +801,7 @@ int hydro_set_limiter(hydro_t* h, int enable) {
     if (!h) return HYDRO_EINVAL;
     if (enable && h->prec != 64) return HYDRO_EINVAL;                  // delta = 1e-8 E is below fp32 resolution
     h->limiter = enable ? 1 : 0;
+    drop_graph(h);
     return HYDRO_OK;
 }
 
@@ -679,13 +816,17 @@ int hydro_get_limited_faces(hydro_t* h, long long* n) {
 
 int hydro_set_deposit_width(hydro_t* h, double sigma) {
     if (!h || !(sigma >= 0.0) || !std::isfinite(sigma)) return HYDRO_EINVAL;
+    if (is_slab(h) && deposit_radius(h, sigma) > 4) return HYDRO_EINVAL;          // see hydro_set_slab
     h->sigma = sigma;
+    drop_graph(h);
     return HYDRO_OK;
 }
 
 int hydro_set_step(hydro_t* h, long long step) {
     if (!h || step < 0) return HYDRO_EINVAL;
     h->step = step;
+    CK(cudaMemcpyAsync(&h->diag->step, &h->step, sizeof(long long), cudaMemcpyHostToDevice, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
     return HYDRO_OK;
 }
 

@@ -16,16 +16,20 @@ namespace hydro_dev {
 constexpr int MAX_JETS = 64;
 
 // ------------------------------------------------------------------------------------------------ diagnostics
-// One slot per "generation" of primitives (two alternate): k_prim fills a slot for the state it converts,
-// k_source commits it to the totals when a stage actually consumes that state.
+// One slot per "generation" of primitives (three rotate, one per stage of an RK3 step, so that every step uses the
+// same sequence and one step can be replayed as a CUDA graph): k_prim fills a slot for the state it converts,
+// k_source commits it to the totals when a stage actually consumes that state and clears the slot the NEXT k_prim
+// will fill.
 struct DiagSlot {
     unsigned long long alpha_bits[3];   // max wavespeed per direction, as the bit pattern of a non-negative real
     unsigned long long ncap;            // cells where the floor / cap of con2prim fired
     unsigned long long nan_flag;        // a non-finite conserved value was seen
     unsigned long long pad[3];
 };
+constexpr int NSLOT = 3;
 struct Diag {
-    DiagSlot slot[2];
+    DiagSlot slot[NSLOT];
+    long long step;                     // completed RK3 steps (device copy: jet positions of a replayed graph come from here)
     unsigned long long ncap_total;
     unsigned long long nan_total;
     unsigned long long nlim_total;      // limiter (R16): faces with theta < 1, all stages
@@ -137,8 +141,9 @@ struct PrimArgs {
     Diag* diag;
     int slot;
     int nx, nxp;       // cells per row, row pitch
-    long long N, Np;   // interior cells, field stride
+    long long c0, N, Np;   // interior cells [c0, N) of this launch (a range of z planes), field stride
     long long own_lo, own_hi;   // cap events are counted for interior cells in [own_lo, own_hi) only (slab halos excluded)
+    int with_alpha;    // 0: primitives only (halo planes of a z-slab: their speeds are the neighbour's business)
     R e_floor, one_minus_delta;
 };
 
@@ -182,7 +187,7 @@ __global__ void __launch_bounds__(256, 4) k_prim(PrimArgs<R> a) {
         am[2] = lz > am[2] ? lz : am[2];
     };
     // two cells per trip: eight independent loads in flight per thread before the arithmetic starts
-    long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    long long c = a.c0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;
     for (; c + stride < a.N; c += 2 * stride) {
         const long long p1 = pad_index(c, a.nx, a.nxp), p2 = pad_index(c + stride, a.nx, a.nxp);
         const R E = U0[p1], Mx = U1[p1], My = U2[p1], Mz = U3[p1];
@@ -222,7 +227,7 @@ __global__ void __launch_bounds__(256, 4) k_prim(PrimArgs<R> a) {
             r[4] |= sm[w][4];
         }
         DiagSlot* s = &a.diag->slot[a.slot];
-        for (int d = 0; d < 3; ++d) atomicMax(&s->alpha_bits[d], r[d]);
+        if (a.with_alpha) for (int d = 0; d < 3; ++d) atomicMax(&s->alpha_bits[d], r[d]);
         if (r[3]) atomicAdd(&s->ncap, r[3]);
         if (r[4]) atomicOr(&s->nan_flag, 1ull);
     }
@@ -339,9 +344,11 @@ struct SourceArgs {
     Diag* diag;
     const JetDev* jets;
     int njets, slot, stage, commit;    // commit: add the slot's cap/NaN counts to the totals, log q, accumulate deposits
+    int zero_slot;                     // >= 0: clear this DiagSlot (the one the next k_prim fills)
+    int advance;                       // 1: this is the last stage of a step: diag->step += 1 afterwards
     int nx, ny, nz, nxp;
     int nz_global, k_offset, own_lo, own_hi;   // z-slab (f-4): global planes, global index of local plane 0, owned local planes
-    long long N /* field stride Np */, step;
+    long long N /* field stride Np */;
     double stage_c, dx, dt, rk_weight;
     double scale;                      // the deposit is added to `target` times this (1 for L, b dt for a stage state)
     double sigma;                      // Gaussian deposit width [fm] (R15); 0 = point deposit (R7)
@@ -368,7 +375,16 @@ __global__ void __launch_bounds__(SOURCE_THREADS) k_source(SourceArgs a, const R
     __shared__ int sh_c[3];
     const int tid = threadIdx.x;
     Diag* dg = a.diag;
+    const long long step = dg->step;                                 // read by every thread before thread 0 advances it
+    __syncthreads();
     if (tid == 0) {
+        if (a.zero_slot >= 0) {
+            DiagSlot* z = &dg->slot[a.zero_slot];
+            z->alpha_bits[0] = z->alpha_bits[1] = z->alpha_bits[2] = 0ull;
+            z->ncap = 0ull;
+            z->nan_flag = 0ull;
+        }
+        if (a.advance) dg->step = step + 1;
         const DiagSlot* s = &dg->slot[a.slot];
 #pragma unroll
         for (int d = 0; d < 3; ++d) dg->alpha_last[d] = (double)Real<R>::from_bits(s->alpha_bits[d]);
@@ -383,7 +399,7 @@ __global__ void __launch_bounds__(SOURCE_THREADS) k_source(SourceArgs a, const R
     for (int J = 0; J < a.njets; ++J) {
         const JetDev jt = a.jets[J];
         if (tid == 0) {
-            const double ell = __dmul_rn(__dadd_rn((double)(a.step - jt.step_added), a.stage_c), a.dt);
+            const double ell = __dmul_rn(__dadd_rn((double)(step - jt.step_added), a.stage_c), a.dt);
             const double xj = __dadd_rn(jt.x0, __dmul_rn(jt.nx, ell)), yj = __dadd_rn(jt.y0, __dmul_rn(jt.ny, ell)),
                          zj = __dadd_rn(jt.z0, __dmul_rn(jt.nz, ell));
             const int ci = jet_axis_index(xj, a.nx, a.dx);
@@ -392,7 +408,8 @@ __global__ void __launch_bounds__(SOURCE_THREADS) k_source(SourceArgs a, const R
             if (ck >= 0) { ck -= a.k_offset; if (ck >= a.nz) ck = -1; }        // global -> local plane; outside the local array: no deposit here
             const bool owned = ck >= a.own_lo && ck < a.own_hi;
             double q = 0.0;
-            if (ci >= 0 && cj >= 0 && ck >= 0) {
+            // a point deposit into a halo plane would be overwritten by the next exchange: skipped (its P may be stale)
+            if (ci >= 0 && cj >= 0 && ck >= 0 && (owned || a.sigma > 0.0)) {
                 const long long c = ((long long)ck * a.ny + cj) * a.nxp + ci;
                 const double e_c = 3.0 * (double)P[c];
                 const double T2 = sqrt(e_c / (G_DOF * HBARC));       // T^2, T in 1/fm

@@ -127,6 +127,8 @@ struct RingArgs {
     double dt, rk_a, rk_b;
     double k3lam;              // limiter: 3 dt/dx (6 dt/dx times the correction C = corr/2 carried as 2 F_hat)
     unsigned long long* nlim;  // limiter: count of faces with theta < 1
+    int own_lo, own_hi;        // limiter count: only faces of owned planes (z sweep: faces whose LOWER cell is owned, and the
+                               // physical boundary face below plane 0), so that sums over ranks are global figures
 };
 
 // element offset inside a sub-tile of march row r (0..7) for this lane
@@ -649,7 +651,8 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
                 __syncthreads();
                 if (f == 0) {
                     const int n1 = theta_row<7, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, (R)a.k3lam);
-                    if (s0 == 0) nlim_local += n1;                     // inner segment starts are counted by the segment before
+                    // inner segment starts are counted by the segment before; z sweep: the face below plane 0
+                    if (s0 == 0 && (DIR == 2 ? a.own_lo == 0 : (tfix >= a.own_lo && tfix < a.own_hi))) nlim_local += n1;
                 }
                 __syncthreads();
                 cx.fhat_prev = tht[sub_off<DIR, R>(7, lane)] * corr;
@@ -662,17 +665,23 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
             mbar_wait(&full_ul[m & 1], (m >> 1) & 1);
             __syncthreads();
             const R k3 = (R)a.k3lam;
+            // faces of rows 2f, 2f+1: lower cells cm + 2f - 4, cm + 2f - 3
+            const int il = cm + 2 * f - 4;
+            const bool cnt0 = DIR == 2 ? (il >= a.own_lo && il < a.own_hi) : (tfix >= a.own_lo && tfix < a.own_hi);
+            const bool cnt1 = DIR == 2 ? (il + 1 >= a.own_lo && il + 1 < a.own_hi) : cnt0;
+            int n0 = 0, n1 = 0;
             switch (f) {
-                case 0: nlim_local += theta_row<0, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3) +
-                                      theta_row<1, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3); break;
-                case 1: nlim_local += theta_row<2, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3) +
-                                      theta_row<3, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3); break;
-                case 2: nlim_local += theta_row<4, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3) +
-                                      theta_row<5, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3); break;
-                case 3: nlim_local += theta_row<6, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3) +
-                                      theta_row<7, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3); break;
+                case 0: n0 = theta_row<0, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3);
+                        n1 = theta_row<1, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3); break;
+                case 1: n0 = theta_row<2, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3);
+                        n1 = theta_row<3, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3); break;
+                case 2: n0 = theta_row<4, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3);
+                        n1 = theta_row<5, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3); break;
+                case 3: n0 = theta_row<6, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3);
+                        n1 = theta_row<7, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3); break;
                 default: break;
             }
+            nlim_local += (cnt0 ? n0 : 0) + (cnt1 ? n1 : 0);
             __syncthreads();
             cx.template emit_lim<0>(); cx.template emit_lim<1>(); cx.template emit_lim<2>(); cx.template emit_lim<3>();
             cx.template emit_lim<4>(); cx.template emit_lim<5>(); cx.template emit_lim<6>(); cx.template emit_lim<7>();

@@ -23,7 +23,7 @@ K_NAMES = ("prim", "sweep_x", "sweep_y", "sweep_z", "source")
 
 # every symbol include/hydro.h declares (tests check that the library exports all of them)
 SYMBOLS = ("hydro_create", "hydro_destroy", "hydro_set_state", "hydro_add_jet", "hydro_clear_jets", "hydro_set_step", "hydro_set_deposit_width", "hydro_set_limiter", "hydro_get_limited_faces", "hydro_set_slab", "hydro_stage_prims",
-           "hydro_stage_alpha", "hydro_stage_sweeps", "hydro_halo", "hydro_halo_reals", "hydro_step",
+           "hydro_stage_alpha", "hydro_stage_sweeps", "hydro_stage_prims_part", "hydro_stage_sweeps_part", "hydro_stage_alpha_dev", "hydro_halo", "hydro_halo_reals", "hydro_step",
            "hydro_synchronize", "hydro_get_fields", "hydro_eval_rhs", "hydro_get_diag", "hydro_get_last_stage_q",
            "hydro_set_profiling", "hydro_get_kernel_times", "hydro_launch_count", "hydro_sweep_path", "hydro_measure_alu_peak",
            "hydro_strerror", "hydro_last_cuda_error")
@@ -51,11 +51,18 @@ def load():
     try:                                   # (re)build in-tree if the library is missing or older than its sources
         from . import build as _build
         _build.build()
-    except Exception as e:                 # no nvcc, or a compile error: fail loudly below if there is nothing to load
+    except Exception as e:                 # no nvcc, or a compile error
         if not os.path.exists(LIB_PATH):
             raise ImportError("CUDA library %s is missing and could not be built (%s): run "
                               "`python -m paper_1511_02137_b200.build` (there is no CPU fallback)" % (LIB_PATH, e))
+        if any(os.path.getmtime(LIB_PATH) < os.path.getmtime(d) for d in _build.DEPS):
+            raise ImportError("CUDA library %s is older than its sources and the rebuild failed (%s): a stale binary "
+                              "must not run against newer headers" % (LIB_PATH, e))
     L = C.CDLL(LIB_PATH)
+    missing = [n for n in SYMBOLS if not hasattr(L, n)]
+    if missing:
+        raise ImportError("%s does not export %s: rebuild it (python -m paper_1511_02137_b200.build --force)" %
+                          (LIB_PATH, ", ".join(missing)))
     vp, i, d, ll = C.c_void_p, C.c_int, C.c_double, C.c_longlong
     dp = C.POINTER(C.c_double)
     L.hydro_create.restype = i
@@ -78,6 +85,12 @@ def load():
     L.hydro_stage_alpha.argtypes = [vp, i, i, dp]
     L.hydro_stage_sweeps.restype = i
     L.hydro_stage_sweeps.argtypes = [vp, i]
+    L.hydro_stage_prims_part.restype = i
+    L.hydro_stage_prims_part.argtypes = [vp, i, i]
+    L.hydro_stage_sweeps_part.restype = i
+    L.hydro_stage_sweeps_part.argtypes = [vp, i, i]
+    L.hydro_stage_alpha_dev.restype = i
+    L.hydro_stage_alpha_dev.argtypes = [vp, i, i, vp]
     L.hydro_halo.restype = i
     L.hydro_halo.argtypes = [vp, i, i, i, vp]
     L.hydro_halo_reals.restype = ll
@@ -223,6 +236,18 @@ class Hydro:
 
     def stage_sweeps(self, s):
         self._ck(self.L.hydro_stage_sweeps(self.h, s), "hydro_stage_sweeps")
+
+    def stage_prims_part(self, s, part):
+        self._ck(self.L.hydro_stage_prims_part(self.h, s, part), "hydro_stage_prims_part")
+
+    def stage_sweeps_part(self, s, part):
+        self._ck(self.L.hydro_stage_sweeps_part(self.h, s, part), "hydro_stage_sweeps_part")
+
+    def stage_alpha_dev(self, s, bits, set=False):
+        """bits: CUDA int64 tensor of 3 elements (the alpha bit patterns); asynchronous on the handle's stream."""
+        assert bits.is_cuda and bits.numel() >= 3 and bits.element_size() == 8
+        self._ck(self.L.hydro_stage_alpha_dev(self.h, s, 1 if set else 0, C.c_void_p(bits.data_ptr())),
+                 "hydro_stage_alpha_dev")
 
     def halo(self, s, side, unpack, buf):
         """buf: CUDA torch tensor of halo_reals() elements of the handle's dtype."""

@@ -176,6 +176,25 @@ def test_config0_five_fields_and_ragged_grid(H, oracle):
     g.close(), o.close()
 
 
+def test_five_fields_multi_wave_grid(H, oracle):
+    """nf = 5 on a grid whose three sweeps each launch more tiles than resident block slots (several waves + the
+    tail-split last wave of hydro.cu launch_ring_nf): one evaluation of L(U) (OUT_STORE / OUT_REDUCE kernels) and a
+    2-step run (OUT_COMBINE kernels) against the oracle on every cell."""
+    c = S.scaled_config(3, (136, 168, 130))
+    c["nf"] = 5
+    c["jets"] = [((-5.0, 0.0, 0.0), (1.0, 0.0, 0.0)), ((1.0, 2.0, -1.0), (-1.0, 1.0, 0.5))]
+    c, U0, g, o = make_pair(H, oracle, c)
+    Lg, Lo = g.eval_rhs(0.5), o.eval_rhs(0.5)
+    scale = np.max(np.abs(Lo), axis=(1, 2, 3))
+    for f in range(5):
+        assert np.max(np.abs(Lg[f] - Lo[f])) <= TOL_STAGE * max(scale[f], scale[0]), f
+    g.step(2), o.step(2)
+    errs = r13(g.get_fields(), o.get_fields())
+    assert max(errs) < TOL_RUN, errs
+    compare_diag(g, o, 2)
+    g.close(), o.close()
+
+
 def test_config1_shock_tube(H, oracle):
     """BASELINE config 1: 512x8x8, 375 steps; GPU vs oracle, and GPU vs the exact Riemann solution (pin P4)."""
     from test_oracle_riemann import exact_solution, exact_profile
@@ -450,7 +469,7 @@ def test_smeared_deposit_run(H, oracle, prec, tol):
 
 
 # ------------------------------------------------------------------------------------------------ flux limiter (f-1)
-def _rough_state(n, seed, vmax=0.98):
+def _rough_state(n, seed, vmax=0.98, nf=4):
     rng = np.random.default_rng(seed)
     shape = (n[2], n[1], n[0])
     e = 10.0 ** rng.uniform(-2, 2, shape)
@@ -458,31 +477,34 @@ def _rough_state(n, seed, vmax=0.98):
     d = rng.normal(size=(3,) + shape)
     d /= np.linalg.norm(d, axis=0)
     u = vm / np.sqrt(1 - vm * vm) * d
-    return S.prim_to_cons(e, u[0], u[1], u[2])
+    return S.prim_to_cons(e, u[0], u[1], u[2], e / 10.0 if nf == 5 else None)
 
 
 @pytest.mark.parametrize("n", [(32, 32, 32), (37, 19, 23), (9, 5, 3), (72, 12, 40)])
 @pytest.mark.parametrize("order", [7, 5])
-def test_limiter_rhs_parity(H, oracle, n, order):
+@pytest.mark.parametrize("nf", [4, 5])
+def test_limiter_rhs_parity(H, oracle, n, order, nf):
     """R16 on rough admissible data (the limiter acts on a large share of the faces) and on smooth data with a jet:
-    L of the limited scheme, GPU vs oracle."""
+    L of the limited scheme, GPU vs oracle; nf = 5 is BASELINE config 4's field count (the baryon density is limited with
+    the same theta as the energy-momentum fields)."""
     for kind in ("rough", "smooth"):
         if kind == "rough":
-            U0 = _rough_state(n, 5)
+            U0 = _rough_state(n, 5, nf=nf)
             jets = []
         else:
             c = S.scaled_config(0, n)
+            c["nf"] = nf
             U0 = S.make_state(c)
             jets = [((-0.12, 0.03, 0.0), (1.0, 0.5, -0.25))]
-        g = H.Hydro(*n, 0.1, 0.02, weno_order=order)
-        o = oracle.Oracle(*n, 0.1, 0.02, weno_order=order)
+        g = H.Hydro(*n, 0.1, 0.02, weno_order=order, nfields=nf)
+        o = oracle.Oracle(*n, 0.1, 0.02, weno_order=order, nfields=nf)
         g.set_state(U0), o.set_state(U0)
         g.set_limiter(True), o.set_limiter(True)
         for pos, d in jets:
             g.add_jet(pos, d), o.add_jet(pos, d)
         Lg, Lo = g.eval_rhs(0.5), o.eval_rhs(0.5)
         scale = np.max(np.abs(Lo), axis=(1, 2, 3))
-        for f in range(4):
+        for f in range(nf):
             # L is recovered from the limited Euler update: (U' - U)/dt costs ulp(U)/dt of absolute accuracy
             tol = 1e-11 * max(scale[f], scale[0]) + 4e-16 * np.max(np.abs(U0[f])) / 0.02
             assert np.max(np.abs(Lg[f] - Lo[f])) <= tol, (kind, f)
@@ -492,6 +514,25 @@ def test_limiter_rhs_parity(H, oracle, n, order):
         else:
             assert ng == no == 0
         g.close(), o.close()
+
+
+def test_limiter_run_five_fields(H, oracle):
+    """Limiter x nf = 5 over a run (the jet/cap case with a baryon density): parity, no cap events, N_B limited too."""
+    c = S.scaled_config(2, (64, 32, 32))
+    c["nf"] = 5
+    c["jets"] = [((-2.0, 0.0, 0.0), (1.0, 0.0, 0.0))]
+    steps = 40
+    c, U0, g, o = make_pair(H, oracle, c)
+    g.set_limiter(True), o.set_limiter(True)
+    g.step(steps), o.step(steps)
+    Ug, Uo = g.get_fields(), o.get_fields()
+    errs = r13(Ug, Uo)
+    assert max(errs) < 1e-8, errs
+    dg, do = compare_diag(g, o, steps)
+    assert dg["ncap"] == do["ncap"] == 0
+    ng, no = g.limited_faces(), o.limited_faces()
+    assert no > 0 and abs(ng - no) <= max(3, 0.02 * no)
+    g.close(), o.close()
 
 
 def test_limiter_runs(H, oracle):
@@ -573,6 +614,36 @@ def test_device_pointers_and_streams(H, oracle):
     assert np.array_equal(out.cpu().numpy(), g2.get_fields())
     assert g.launch_count() == 2 * (3 * 5) + 1
     g.close(), g2.close()
+
+
+def test_graph_replay_equals_individual_launches(H):
+    """hydro_step replays one captured RK3 step as a CUDA graph (the step counter lives on the device); with per-kernel
+    profiling on it launches the 15 kernels one by one.  Same kernels, same arguments: bitwise equal states, equal
+    diagnostics and launch counts, across split calls, a jet added mid-run (recapture) and set_step."""
+    c = S.scaled_config(0, (40, 24, 20))
+    U0 = S.make_state(c)
+    out = []
+    for profiled in (False, True):
+        g = H.Hydro(*c["n"], c["dx"], c["dt"])
+        g.set_state(U0)
+        g.set_profiling(profiled)
+        g.add_jet((-1.0, 0.0, 0.0), (1.0, 0.0, 0.0))
+        g.step(3)
+        g.step(1)
+        g.add_jet((0.3, 0.2, -0.1), (0.0, 1.0, 0.5))
+        g.step(4)
+        g.set_deposit_width(0.1)
+        g.step(2)
+        g.set_step(20)
+        g.step(2)
+        d = g.diag()
+        out.append((g.get_fields(), d, g.last_stage_q(), g.launch_count()))
+        g.close()
+    (Ua, da, qa, la), (Ub, db, qb, lb) = out
+    assert np.array_equal(Ua, Ub) and la == lb
+    assert da["step"] == db["step"] == 22 and da["ncap"] == db["ncap"]
+    assert np.array_equal(da["deposited"], db["deposited"]) and np.array_equal(da["alpha"], db["alpha"])
+    assert np.array_equal(qa, qb)
 
 
 def test_checkpoint_resume_is_bitwise(H):
