@@ -125,7 +125,7 @@ struct RingArgs {
     double eps_eff;            // WENO7: 144 * weno_eps (the split fluxes are carried as 2 f^+-, beta as 36 beta); WENO5: 48 * weno_eps
     double coef;               // OUT_STORE / OUT_REDUCE: c = [b dt] / (2 dx);  OUT_COMBINE*: 1 / (2 dx)
     double dt, rk_a, rk_b;
-    double k3lam;              // limiter: 3 dt/dx (6 dt/dx times the correction C = corr/2 carried as 2 F_hat)
+    double k3lam;              // limiter: 6 dt/dx times the correction C = corr / (2 KW) (the exchange tile holds corr = KW x 2 C)
     unsigned long long* nlim;  // limiter: count of faces with theta < 1
     int own_lo, own_hi;        // limiter count: only faces of owned planes (z sweep: faces whose LOWER cell is owned, and the
                                // physical boundary face below plane 0), so that sums over ranks are global figures
@@ -146,8 +146,20 @@ __device__ __forceinline__ int sub_off(int r, int lane) {
 
 // ------------------------------------------------------------------------------------------------ rotating window
 // Undivided differences of one split flux along the march, slot = march row mod 8:
-//   V = value, D = V - V_prev, E = D - D_prev, T = E - E_prev (only the newest is kept), G = T - T_prev,
-//   S = C3 T^2 + eps.  Live at any time: 4 V, 6 D, 5 E, 4 S, 3 G, 1 T (the other slots are dead registers).
+//   V = value, D = V - V_prev, E = sE (D - D_prev), T = E - E_prev (only the newest is kept), G = T - T_prev,
+//   S = cT T^2 + eps.  Live at any time: 4 V, 6 D, 5 E, 4 S, 3 G, 1 T (the other slots are dead registers).
+// The second differences and everything derived from them (T, G) are carried SCALED by sE = sqrt(39) (WENO7) or
+// sqrt(13) (WENO5): the smoothness indicators need 39 m^2 (13 E^2), so the scaled values enter them as plain squares --
+// one multiplication per cell instead of three per reconstruction; the linear uses of G and m fold 1/sE into FMA constants.
+template <int ORDER> struct WinScale;
+template <> struct WinScale<7> {
+    static constexpr double sE = 6.2449979983983982058, iE = 0.16012815380508713318;      // sqrt(39), 1/sqrt(39)
+    static constexpr double cT = 39.05 / 39.0;                                            // 39.05 T^2 = cT (sE T)^2
+};
+template <> struct WinScale<5> {
+    static constexpr double sE = 3.6055512754639892931, iE = 0.27735009811261456101;      // sqrt(13), 1/sqrt(13)
+    static constexpr double cT = 0.0;
+};
 template <typename R>
 struct RotWin {
     R V[8], D[8], E[8], S[8], G[8], T;
@@ -159,14 +171,14 @@ struct RotWin {
 };
 
 template <int r, int ORDER, typename R>
-__device__ __forceinline__ void rot_push(RotWin<R>& w, R x, R c3, R eps) {
+__device__ __forceinline__ void rot_push(RotWin<R>& w, R x, R eps) {
     constexpr int p = (r + 7) & 7;
     const R dn = x - w.V[p];
-    const R en = dn - w.D[p];
+    const R en = R(WinScale<ORDER>::sE) * (dn - w.D[p]);
     if (ORDER == 7) {
         const R tn = en - w.E[p];
         w.G[r] = tn - w.T;
-        w.S[r] = Real<R>::fma_(c3 * tn, tn, eps);
+        w.S[r] = Real<R>::fma_(R(WinScale<7>::cT) * tn, tn, eps);
         w.T = tn;
     }
     w.V[r] = x;
@@ -189,30 +201,30 @@ __device__ __forceinline__ float rcp_ulp(float x) {      // MUFU.RCP: 1 ulp, eno
     return r;
 }
 
-// One WENO7-JS reconstruction (r = 4) from the 1st..4th undivided differences in stencil order (D_j, E_j, G_j) and
-// S_j = 39.05 T_j^2 + eps (formulas: DESIGN.md "WENO7 in difference form"):
+// One WENO7-JS reconstruction (r = 4) from the 1st..4th undivided differences in stencil order (D_j; E_j, G_j scaled by
+// sE = sqrt(39), see RotWin) and S_j = 39.05 T_j^2 + eps (formulas: DESIGN.md "WENO7 in difference form"):
 //   candidates   12 (q_0 - x_c) = 3 D_0 - 10 D_1 + 13 D_2,  12 (q_1-q_0) = 3 G_0,  12 (q_2-q_1) = -G_1,  12 (q_3-q_2) = G_2
 //   smoothness   36 beta_k + eps = lam_k^2 + 39 m_k^2 + S_k,
 //                lam_0 = 2 D_0 - 7 D_1 + 11 D_2, lam_1 = lam_0 + 2 G_0, lam_2 = lam_1 - G_1, lam_3 = lam_2 + 2 G_2,
 //                m_0 = 2 E_1 - E_0,  m_1 = m_2 = E_2,  m_3 = 2 E_3 - E_4
 //   weights      fp64: omega_k ~ d_k prod_{j != k} (eps + beta_j)^2,  d = (1, 12, 18, 4)/35  (common denominator;
 //                range-safe in fp64);  fp32: omega_k ~ d_k (1/(eps + beta_k))^2, one reciprocal each (R10)
-// Returns base12 = 12 (q_0 - x_c) and num12/den = 12 sum_k omega_k (q_k - q_0):  W = x_c + (base12 + num12/den)/12.
+// Returns base12 = 12 (q_0 - x_c) and num12s/den = sE 12 sum_k omega_k (q_k - q_0):  W = x_c + (base12 + num12s/(sE den))/12.
 template <typename R>
 __device__ __forceinline__ void weno7_diff(R D0, R D1, R D2, R E0, R E1, R E2, R E3, R E4, R S0, R S1, R S2, R S3,
-                                           R G0, R G1, R G2, R& base12, R& num12, R& den) {
+                                           R G0, R G1, R G2, R& base12, R& num12s, R& den) {
     typedef Real<R> T;
+    constexpr double iE = WinScale<7>::iE;
     const R lam0 = T::fma_(R(11), D2, T::fma_(R(-7), D1, R(2) * D0));
-    const R lam1 = T::fma_(R(2), G0, lam0);
-    const R lam2 = lam1 - G1;
-    const R lam3 = T::fma_(R(2), G2, lam2);
-    const R m0 = T::fma_(R(2), E1, -E0);
+    const R lam1 = T::fma_(R(2 * iE), G0, lam0);
+    const R lam2 = T::fma_(R(-iE), G1, lam1);
+    const R lam3 = T::fma_(R(2 * iE), G2, lam2);
+    const R m0 = T::fma_(R(2), E1, -E0);                  // sE m_0, sE m_3: their squares are 39 m^2
     const R m3 = T::fma_(R(2), E3, -E4);
-    const R e39 = R(39) * E2;
-    const R b0 = T::fma_(lam0, lam0, T::fma_(R(39) * m0, m0, S0));
-    const R b1 = T::fma_(lam1, lam1, T::fma_(e39, E2, S1));
-    const R b2 = T::fma_(lam2, lam2, T::fma_(e39, E2, S2));
-    const R b3 = T::fma_(lam3, lam3, T::fma_(R(39) * m3, m3, S3));
+    const R b0 = T::fma_(lam0, lam0, T::fma_(m0, m0, S0));
+    const R b1 = T::fma_(lam1, lam1, T::fma_(E2, E2, S1));
+    const R b2 = T::fma_(lam2, lam2, T::fma_(E2, E2, S2));
+    const R b3 = T::fma_(lam3, lam3, T::fma_(m3, m3, S3));
     R u0, u1, u2, u3;
     if (sizeof(R) == 8) {
         const R t0 = b0 * b0, t1 = b1 * b1, t2 = b2 * b2, t3 = b3 * b3;
@@ -226,25 +238,25 @@ __device__ __forceinline__ void weno7_diff(R D0, R D1, R D2, R E0, R E1, R E2, R
     const R a23 = T::fma_(R(18), u2, a3);
     const R a123 = T::fma_(R(12), u1, a23);
     den = u0 + a123;
-    num12 = T::fma_(a123, R(3) * G0, T::fma_(-a23, G1, a3 * G2));
-    base12 = lam0 + m0;                                   // 3 D_0 - 10 D_1 + 13 D_2 = lam_0 + m_0 identically
+    num12s = T::fma_(a123, R(3) * G0, T::fma_(-a23, G1, a3 * G2));
+    base12 = T::fma_(R(iE), m0, lam0);                    // 3 D_0 - 10 D_1 + 13 D_2 = lam_0 + m_0 identically
 }
 
 // One WENO5-JS reconstruction (r = 3) from the differences of the stencil values
-// x_0..x_4 (centre x_2), D_j = x_{j+1} - x_j, E_j = D_{j+1} - D_j:
+// x_0..x_4 (centre x_2), D_j = x_{j+1} - x_j, E_j = D_{j+1} - D_j (carried scaled by sE = sqrt(13), see RotWin):
 //   candidates   6 (q_0 - x_2) = 5 D_1 - 2 D_0,   6 (q_1 - q_0) = 2 (E_1 - E_0),   6 (q_2 - q_1) = -(E_2 - E_1)
 //   smoothness   12 beta_k + eps = 13 E_k^2 + 3 l_k^2 + eps,  l_0 = 3 D_1 - D_0,  l_1 = D_1 + D_2,  l_2 = 3 D_2 - D_3
 //   weights      omega_k ~ d_k / (eps + beta_k)^2,  d = (1, 6, 3)/10  (fp64: common denominator; fp32: reciprocals)
-// Returns base6 = 6 (q_0 - x_2) and num6/den = 6 sum_k omega_k (q_k - q_0):  W = x_2 + (base6 + num6/den)/6.
+// Returns base6 = 6 (q_0 - x_2) and num6s/den = sE 6 sum_k omega_k (q_k - q_0):  W = x_2 + (base6 + num6s/(sE den))/6.
 template <typename R>
-__device__ __forceinline__ void weno5_diff(R D0, R D1, R D2, R D3, R E0, R E1, R E2, R eps, R& base6, R& num6, R& den) {
+__device__ __forceinline__ void weno5_diff(R D0, R D1, R D2, R D3, R E0, R E1, R E2, R eps, R& base6, R& num6s, R& den) {
     typedef Real<R> T;
     const R l0 = T::fma_(R(3), D1, -D0);
     const R l1 = D1 + D2;
     const R l2 = T::fma_(R(3), D2, -D3);
-    const R b0 = T::fma_(R(13) * E0, E0, T::fma_(R(3) * l0, l0, eps));
-    const R b1 = T::fma_(R(13) * E1, E1, T::fma_(R(3) * l1, l1, eps));
-    const R b2 = T::fma_(R(13) * E2, E2, T::fma_(R(3) * l2, l2, eps));
+    const R b0 = T::fma_(E0, E0, T::fma_(R(3) * l0, l0, eps));
+    const R b1 = T::fma_(E1, E1, T::fma_(R(3) * l1, l1, eps));
+    const R b2 = T::fma_(E2, E2, T::fma_(R(3) * l2, l2, eps));
     R u0, u1, u2;
     if (sizeof(R) == 8) {
         const R t0 = b0 * b0, t1 = b1 * b1, t2 = b2 * b2;
@@ -256,7 +268,7 @@ __device__ __forceinline__ void weno5_diff(R D0, R D1, R D2, R D3, R E0, R E1, R
     const R a2 = R(3) * u2;
     const R a12 = T::fma_(R(6), u1, a2);
     den = u0 + a12;
-    num6 = T::fma_(a12, R(2) * (E1 - E0), -a2 * (E2 - E1));
+    num6s = T::fma_(a12, R(2) * (E1 - E0), -a2 * (E2 - E1));
     base6 = T::fma_(R(5), D1, R(-2) * D0);
 }
 
@@ -264,8 +276,8 @@ __device__ __forceinline__ void weno5_diff(R D0, R D1, R D2, R D3, R E0, R E1, R
 //   plus  side: cells i-3..i+3 = slots r-7..r-1, centre i   = V[r-4]
 //   minus side: cells i-2..i+4 = slots r-6..r,   centre i+1 = V[r-3], stencil order reversed (D_j = -d[5-j], ...)
 //   ORDER 5: plus cells i-2..i+2 = slots r-6..r-2 (centre V[r-4]); minus cells i-1..i+3 = slots r-5..r-1 reversed
-// rot_flux_parts: 2 F_hat = vsum + corr with vsum = 2 f+_i + 2 f-_{i+1} (twice the first-order Lax-Friedrichs flux) and
-// corr the high-order WENO correction (the limiter of R16 scales corr by theta).
+// rot_flux_parts: 2 F_hat = vsum + corr / KW (KW = 12 for WENO7, 6 for WENO5) with vsum = 2 f+_i + 2 f-_{i+1} (twice the
+// first-order Lax-Friedrichs flux) and corr / KW the high-order WENO correction (the limiter of R16 scales it by theta).
 template <int r, int ORDER, typename R>
 __device__ __forceinline__ void rot_flux_parts(const RotWin<R>& wp, const RotWin<R>& wm, R eps, R& vsum, R& corr) {
 #define SL(k) (((r) + (k) + 16) & 7)
@@ -285,18 +297,20 @@ __device__ __forceinline__ void rot_flux_parts(const RotWin<R>& wp, const RotWin
                   wm.S[SL(0)], wm.S[SL(-1)], wm.S[SL(-2)], wm.S[SL(-3)],
                   wm.G[SL(0)], wm.G[SL(-1)], wm.G[SL(-2)], bm, nm, dm);
     }
-    R x;
-    if (sizeof(R) == 8) x = (R)(fma((double)np_, (double)dm, (double)nm * (double)dp) * rcp_cubic((double)dp * (double)dm));
-    else x = (R)fmaf((float)np_, rcp_ulp((float)dp), (float)nm * rcp_ulp((float)dm));
-    corr = ((bp + bm) + x) * (ORDER == 5 ? R(1.0 / 6.0) : R(1.0 / 12.0));
+    // xs = sE (num+/den+ + num-/den-): one reciprocal for both sides in fp64
+    R xs;
+    if (sizeof(R) == 8) xs = (R)(fma((double)np_, (double)dm, (double)nm * (double)dp) * rcp_cubic((double)dp * (double)dm));
+    else xs = (R)fmaf((float)np_, rcp_ulp((float)dp), (float)nm * rcp_ulp((float)dm));
+    corr = Real<R>::fma_(R(WinScale<ORDER>::iE), xs, bp + bm);               // KW x (high-order correction), KW = 12 or 6
     vsum = wp.V[SL(-4)] + wm.V[SL(-3)];
 #undef SL
 }
+// KW x (2 F_hat) = KW vsum + corr, KW = 12 (WENO7) or 6 (WENO5): the 1/KW is folded into the divergence coefficient
 template <int r, int ORDER, typename R>
 __device__ __forceinline__ R rot_flux(const RotWin<R>& wp, const RotWin<R>& wm, R eps) {
     R vsum, corr;
     rot_flux_parts<r, ORDER, R>(wp, wm, eps, vsum, corr);
-    return vsum + corr;
+    return Real<R>::fma_(R(ORDER == 5 ? 6 : 12), vsum, corr);
 }
 
 // per-thread view of one input stage: element pointers with the lane offset folded in
@@ -378,7 +392,7 @@ struct SweepCtx {
     RotWin<R> wp, wm;
     R fhat_prev;
     const R* th;                           // limiter: theta tile
-    R alpha, c3, eps, coef, dt, rk_a, rk_b, kE;
+    R alpha, eps, coef, rk_a, rk_b, kE;       // coef: everything that multiplies (F_hat_prev - F_hat), see the kernel
     // current chunk
     RowPtr<DIR, R> pu, pmd, pa, pw, pp;    // own field, normal momentum, A operand, W (or zeros), P (or zeros)
     RowPtr<DIR, R> pus[2];                 // U_s of the output cells: rows 4..7 of the previous chunk, 0..3 of this one
@@ -404,8 +418,8 @@ struct SweepCtx {
         typedef Real<R> T;
         const R B = T::fma_(in.md, in.w, kE);
         const R F = T::fma_(in.a, B, in.p);
-        rot_push<r, ORDER, R>(wp, T::fma_(alpha, in.u, F), c3, eps);
-        rot_push<r, ORDER, R>(wm, T::fma_(-alpha, in.u, F), c3, eps);
+        rot_push<r, ORDER, R>(wp, T::fma_(alpha, in.u, F), eps);
+        rot_push<r, ORDER, R>(wm, T::fma_(-alpha, in.u, F), eps);
     }
     template <int r>
     __device__ __forceinline__ void load_push() {
@@ -463,15 +477,15 @@ struct SweepCtx {
     template <int r>
     __device__ __forceinline__ void emit_with(const R fhat) {
         typedef Real<R> T;
-        const R mdiv = (fhat_prev - fhat) * coef;
+        const R dlt = fhat_prev - fhat;
         fhat_prev = fhat;
         R o;
-        if (OUT == OUT_STORE || OUT == OUT_REDUCE) o = mdiv;
+        if (OUT == OUT_STORE || OUT == OUT_REDUCE) o = dlt * coef;
         else {
             // output cell i = (row's cell) - 4: U_s from the ring, row (r + 4) & 7 of the previous / this chunk
             const R us = pus[r < 4 ? 0 : 1].template at<(r + 4) & 7>();
-            o = T::fma_(dt, mdiv, us);
-            if (OUT == OUT_COMBINE) o = T::fma_(rk_b, o, rk_a * pun.template at<r>());
+            if (OUT == OUT_COMBINE) o = T::fma_(coef, dlt, T::fma_(rk_b, us, rk_a * pun.template at<r>()));
+            else o = T::fma_(coef, dlt, us);
         }
         out[sub_off<DIR, R>(r, lane)] = o;
     }
@@ -579,10 +593,13 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
     cx.wm.clear();
     cx.fhat_prev = R(0);
     cx.alpha = Real<R>::from_bits(a.diag->slot[a.slot].alpha_bits[DIR]);
-    cx.c3 = R(39.05);
     cx.eps = (R)a.eps_eff;
-    cx.coef = (R)a.coef;
-    cx.dt = (R)a.dt;
+    {
+        // the fluxes are carried as KW x 2 F_hat (KW = 12, 6: rot_flux); c = a.coef / KW turns their difference into the
+        // divergence part; the COMBINE kernels fold dt (and the RK weight b) in: U_next = a U^n + b U_s + (b dt c) (F- - F+)
+        const double c = a.coef / (ORDER == 5 ? 6.0 : 12.0);
+        cx.coef = (R)(OUT == OUT_COMBINE ? a.rk_b * a.dt * c : OUT == OUT_COMBINE1 ? a.dt * c : c);
+    }
     cx.rk_a = (R)a.rk_a;
     cx.rk_b = (R)a.rk_b;
     cx.lane = lane;
