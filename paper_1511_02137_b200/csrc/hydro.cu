@@ -49,6 +49,7 @@ struct hydro {
     bool view;                          // launch the sweeps on the owned-planes view (hydro_stage_sweeps_part)
     int seg_len[3], tma_nseg[3];
     int num_sms;
+    int prim_blocks_per_sm;             // resident k_prim blocks per SM (occupancy query at create)
     long long launches;
     // one RK3 step captured as a CUDA graph (replayed by hydro_step when profiling is off): valid for graph_slot only and
     // until the jets, the limiter, the deposit width or the slab change
@@ -135,14 +136,16 @@ int launch_prim_range(hydro* h, const void* U, int slot, int k0, int k1, bool re
     PrimArgs<R> a;
     a.U = (const R*)U; a.P = (R*)h->P; a.W = (R*)h->W; a.diag = h->diag; a.slot = slot; a.c0 = k0 * plane; a.N = k1 * plane;
     a.Np = h->Np; a.nx = h->nx; a.nxp = h->nxp; a.with_alpha = with_alpha ? 1 : 0;
+    a.seed_slot = (slot + NSLOT - 1) % NSLOT;                       // the previous stage's slot: its arg[] names good candidates
     a.own_lo = (long long)h->own_lo * plane; a.own_hi = (long long)h->own_hi * plane;
     a.e_floor = (R)h->e_floor; a.one_minus_delta = (R)(1.0 - h->delta);
-    long long blocks = (a.N - a.c0 + 255) / 256;
-    long long cap = (long long)h->num_sms * 8;
+    // grid-stride over the range with exactly one wave of resident blocks (no partial last wave)
+    long long blocks = (a.N - a.c0 + PRIM_THREADS - 1) / PRIM_THREADS;
+    long long cap = (long long)h->num_sms * h->prim_blocks_per_sm;
     if (blocks > cap) blocks = cap;
     {
         Timer t(h, HYDRO_K_PRIM);
-        k_prim<R><<<(unsigned)blocks, 256, 0, h->stream>>>(a);
+        k_prim<R><<<(unsigned)blocks, PRIM_THREADS, 0, h->stream>>>(a);
     }
     h->launches += 1;
     CK(cudaGetLastError());
@@ -653,6 +656,10 @@ int hydro_create(hydro_t** out, int nx, int ny, int nz, double dx, double dt, co
         if ((e = cudaMalloc((void**)&h->diag, sizeof(Diag))) != cudaSuccess) { rc = cuda_fail(h, e, "cudaMalloc(diag)"); break; }
         if ((e = cudaMalloc((void**)&h->jets_dev, sizeof(JetDev) * MAX_JETS)) != cudaSuccess) { rc = cuda_fail(h, e, "cudaMalloc(jets)"); break; }
         if ((e = cudaMemsetAsync(h->diag, 0, sizeof(Diag), h->stream)) != cudaSuccess) { rc = cuda_fail(h, e, "cudaMemset(diag)"); break; }
+        h->prim_blocks_per_sm = 0;
+        if (h->prec == 64) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->prim_blocks_per_sm, k_prim<double>, PRIM_THREADS, 0);
+        else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->prim_blocks_per_sm, k_prim<float>, PRIM_THREADS, 0);
+        if (e != cudaSuccess || h->prim_blocks_per_sm < 1) h->prim_blocks_per_sm = 2;
         rc = setup_tma(h);
     } while (0);
     if (rc != HYDRO_OK) {

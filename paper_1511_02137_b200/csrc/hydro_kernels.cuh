@@ -24,7 +24,8 @@ struct DiagSlot {
     unsigned long long alpha_bits[3];   // max wavespeed per direction, as the bit pattern of a non-negative real
     unsigned long long ncap;            // cells where the floor / cap of con2prim fired
     unsigned long long nan_flag;        // a non-finite conserved value was seen
-    unsigned long long pad[3];
+    unsigned long long arg[3];          // interior linear index of a cell whose speed was (close to) the maximum: the
+                                        // NEXT k_prim starts its running maxima from the exact speeds of these cells
 };
 constexpr int NSLOT = 3;
 struct Diag {
@@ -144,6 +145,7 @@ struct PrimArgs {
     long long c0, N, Np;   // interior cells [c0, N) of this launch (a range of z planes), field stride
     long long own_lo, own_hi;   // cap events are counted for interior cells in [own_lo, own_hi) only (slab halos excluded)
     int with_alpha;    // 0: primitives only (halo planes of a z-slab: their speeds are the neighbour's business)
+    int seed_slot;     // DiagSlot whose arg[] names the candidate cells (the previous stage's slot; any slot is valid)
     R e_floor, one_minus_delta;
 };
 
@@ -154,8 +156,26 @@ __device__ __forceinline__ long long pad_index(long long c, int nx, int nxp) {
     return row * nxp + (c - row * nx);
 }
 
+// Exact global maxima without evaluating every cell's speeds: lambda_d of a cell exceeds a threshold M iff
+//     cs sqrt(rad) > M den - |v_d| (1 - cs2)   <=>   t < 0  or  rad / 3 > t^2,   t = M den - |v_d| (1 - cs2),
+// which costs 3 operations instead of a square root, a reciprocal and their Newton steps.  Every thread keeps M_d = the
+// largest speed it has evaluated exactly so far (times 1 - margin, so that rounding in the test can never hide a larger
+// cell) and starts from the exact speeds of three candidate cells of THIS state: the cells that set the maxima of the
+// previous stage's state (DiagSlot::arg) -- true cells of the launch's range, hence lower bounds of the maxima that need
+// no fallback.  Smooth flow: only the warps near the fastest cells ever take the exact path.  The result is the same
+// exact maximum as evaluating every cell (the candidates' owners evaluate them exactly like any other cell).
 template <typename R>
-__global__ void __launch_bounds__(256, 4) k_prim(PrimArgs<R> a) {
+__device__ __forceinline__ void cell_speeds(R Mx, R My, R Mz, R wt, R& vx, R& vy, R& vz, R& om, R& den) {
+    vx = Mx * wt; vy = My * wt; vz = Mz * wt;
+    const R v2 = vx * vx + vy * vy + vz * vz;
+    om = R(1) - v2;
+    om = om < R(0) ? R(0) : om;
+    den = R(1) - v2 * R(1.0 / 3.0);
+}
+
+constexpr int PRIM_THREADS = 256;
+template <typename R>
+__global__ void __launch_bounds__(PRIM_THREADS, 3) k_prim(PrimArgs<R> a) {
     R am[3] = {R(0), R(0), R(0)};
     unsigned int ncap = 0, bad = 0;
     const long long stride = (long long)gridDim.x * blockDim.x;
@@ -163,6 +183,26 @@ __global__ void __launch_bounds__(256, 4) k_prim(PrimArgs<R> a) {
     const R* __restrict__ U1 = a.U + a.Np;
     const R* __restrict__ U2 = a.U + 2 * a.Np;
     const R* __restrict__ U3 = a.U + 3 * a.Np;
+    const R margin = sizeof(R) == 8 ? R(1.0 - 1e-12) : R(1.0 - 1e-5);
+    __shared__ R seed[3];
+    if (a.with_alpha) {
+        if (threadIdx.x < 3) {
+            long long cs = (long long)a.diag->slot[a.seed_slot].arg[threadIdx.x];
+            cs = cs < a.c0 ? a.c0 : (cs > a.N - 1 ? a.N - 1 : cs);
+            const long long pc = pad_index(cs, a.nx, a.nxp);
+            R p, wt, vx, vy, vz, om, den;
+            int lim;
+            con2prim<R>(U0[pc], U1[pc], U2[pc], U3[pc], a.e_floor, a.one_minus_delta, p, wt, lim);
+            cell_speeds<R>(U1[pc], U2[pc], U3[pc], wt, vx, vy, vz, om, den);
+            const R vd = threadIdx.x == 0 ? vx : threadIdx.x == 1 ? vy : vz;
+            const R lam = max_wavespeed<R>(vd, den, Real<R>::rcp_fast(den), om);
+            seed[threadIdx.x] = lam == lam ? lam * margin : R(0);                 // a NaN state: evaluate everything
+        }
+        __syncthreads();
+    }
+    R M[3] = {R(0), R(0), R(0)};
+    long long arg[3] = {a.c0, a.c0, a.c0};
+    if (a.with_alpha) { M[0] = seed[0]; M[1] = seed[1]; M[2] = seed[2]; }
     auto cell = [&](long long c, long long c0, R E, R Mx, R My, R Mz) {
         R p, wt;
         int lim;
@@ -173,20 +213,34 @@ __global__ void __launch_bounds__(256, 4) k_prim(PrimArgs<R> a) {
         // finite check: x - x is 0 for finite x, NaN otherwise
         R chk = (E - E) + (Mx - Mx) + (My - My) + (Mz - Mz);
         bad |= (chk == R(0)) ? 0u : 1u;
-        R vx = Mx * wt, vy = My * wt, vz = Mz * wt;
-        R v2 = vx * vx + vy * vy + vz * vz;
-        R om = R(1) - v2;
-        om = om < R(0) ? R(0) : om;
-        const R den = R(1) - v2 * R(1.0 / 3.0);
-        const R inv_den = Real<R>::rcp_fast(den);
-        R lx = max_wavespeed<R>(vx, den, inv_den, om);
-        R ly = max_wavespeed<R>(vy, den, inv_den, om);
-        R lz = max_wavespeed<R>(vz, den, inv_den, om);
-        am[0] = lx > am[0] ? lx : am[0];
-        am[1] = ly > am[1] ? ly : am[1];
-        am[2] = lz > am[2] ? lz : am[2];
+        if (!a.with_alpha) return;
+        R vx, vy, vz, om, den;
+        cell_speeds<R>(Mx, My, Mz, wt, vx, vy, vz, om, den);
+        const R k23 = R(2.0 / 3.0), k13 = R(1.0 / 3.0);
+        const R tx = Real<R>::fma_(M[0], den, -k23 * (vx < R(0) ? -vx : vx));
+        const R ty = Real<R>::fma_(M[1], den, -k23 * (vy < R(0) ? -vy : vy));
+        const R tz = Real<R>::fma_(M[2], den, -k23 * (vz < R(0) ? -vz : vz));
+        const R rx = k13 * om * Real<R>::fma_(-k23 * vx, vx, den);
+        const R ry = k13 * om * Real<R>::fma_(-k23 * vy, vy, den);
+        const R rz = k13 * om * Real<R>::fma_(-k23 * vz, vz, den);
+        const bool hot = (tx < R(0)) | (rx > tx * tx) | (ty < R(0)) | (ry > ty * ty) | (tz < R(0)) | (rz > tz * tz);
+        if (hot) {                                                   // rare: this cell may raise a maximum
+            const R inv_den = Real<R>::rcp_fast(den);
+            const R lx = max_wavespeed<R>(vx, den, inv_den, om);
+            const R ly = max_wavespeed<R>(vy, den, inv_den, om);
+            const R lz = max_wavespeed<R>(vz, den, inv_den, om);
+            if (lx > am[0]) { am[0] = lx; arg[0] = c0; }
+            if (ly > am[1]) { am[1] = ly; arg[1] = c0; }
+            if (lz > am[2]) { am[2] = lz; arg[2] = c0; }
+            const R mx = lx * margin, my = ly * margin, mz = lz * margin;
+            M[0] = mx > M[0] ? mx : M[0];
+            M[1] = my > M[1] ? my : M[1];
+            M[2] = mz > M[2] ? mz : M[2];
+        }
     };
-    // two cells per trip: eight independent loads in flight per thread before the arithmetic starts
+    // two cells per trip: eight independent loads in flight per thread before the arithmetic starts.  (Tried and measured
+    // slower: issuing the next trip's loads before this trip's arithmetic + L2 prefetch of the trip after, at 128 threads x
+    // 5 blocks: 0.184 ms per launch against 0.166 ms; the loop is bound by load latency at 24 warps/SM, not by the FP64 pipe.)
     long long c = a.c0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;
     for (; c + stride < a.N; c += 2 * stride) {
         const long long p1 = pad_index(c, a.nx, a.nxp), p2 = pad_index(c + stride, a.nx, a.nxp);
@@ -199,7 +253,7 @@ __global__ void __launch_bounds__(256, 4) k_prim(PrimArgs<R> a) {
         const long long p1 = pad_index(c, a.nx, a.nxp);
         cell(p1, c, U0[p1], U1[p1], U2[p1], U3[p1]);
     }
-    // warp reduction by shuffles, then one atomic per warp on the bit pattern (non-negative reals order like
+    // warp reduction by shuffles, then one atomic per block on the bit pattern (non-negative reals order like
     // unsigned integers; the max is exact, hence order independent)
     unsigned long long ab[3];
 #pragma unroll
@@ -208,26 +262,32 @@ __global__ void __launch_bounds__(256, 4) k_prim(PrimArgs<R> a) {
     for (int off = 16; off > 0; off >>= 1) {
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
-            unsigned long long o = __shfl_xor_sync(0xffffffffu, ab[d], off);
-            ab[d] = o > ab[d] ? o : ab[d];
+            const unsigned long long o = __shfl_xor_sync(0xffffffffu, ab[d], off);
+            const long long oa = __shfl_xor_sync(0xffffffffu, arg[d], off);
+            if (o > ab[d]) { ab[d] = o; arg[d] = oa; }
         }
         ncap += __shfl_xor_sync(0xffffffffu, ncap, off);
         bad |= __shfl_xor_sync(0xffffffffu, bad, off);
     }
-    __shared__ unsigned long long sm[8][5];
+    __shared__ unsigned long long sm[8][8];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (lane == 0) { sm[warp][0] = ab[0]; sm[warp][1] = ab[1]; sm[warp][2] = ab[2]; sm[warp][3] = ncap; sm[warp][4] = bad; }
+    if (lane == 0) {
+        sm[warp][0] = ab[0]; sm[warp][1] = ab[1]; sm[warp][2] = ab[2]; sm[warp][3] = ncap; sm[warp][4] = bad;
+        sm[warp][5] = (unsigned long long)arg[0]; sm[warp][6] = (unsigned long long)arg[1]; sm[warp][7] = (unsigned long long)arg[2];
+    }
     __syncthreads();
     if (threadIdx.x == 0) {
-        unsigned long long r[5] = {0, 0, 0, 0, 0};
+        unsigned long long r[5] = {0, 0, 0, 0, 0}, ra[3] = {0, 0, 0};
         const int nw = blockDim.x >> 5;
         for (int w = 0; w < nw; ++w) {
-            for (int d = 0; d < 3; ++d) r[d] = sm[w][d] > r[d] ? sm[w][d] : r[d];
+            for (int d = 0; d < 3; ++d) if (sm[w][d] > r[d]) { r[d] = sm[w][d]; ra[d] = sm[w][5 + d]; }
             r[3] += sm[w][3];
             r[4] |= sm[w][4];
         }
         DiagSlot* s = &a.diag->slot[a.slot];
-        if (a.with_alpha) for (int d = 0; d < 3; ++d) atomicMax(&s->alpha_bits[d], r[d]);
+        if (a.with_alpha)
+            for (int d = 0; d < 3; ++d)
+                if (r[d] && atomicMax(&s->alpha_bits[d], r[d]) < r[d]) s->arg[d] = ra[d];   // the last raiser holds the maximum
         if (r[3]) atomicAdd(&s->ncap, r[3]);
         if (r[4]) atomicOr(&s->nan_flag, 1ull);
     }
