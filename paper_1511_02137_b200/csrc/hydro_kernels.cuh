@@ -238,17 +238,37 @@ __global__ void __launch_bounds__(PRIM_THREADS, 3) k_prim(PrimArgs<R> a) {
             M[2] = mz > M[2] ? mz : M[2];
         }
     };
-    // two cells per trip: eight independent loads in flight per thread before the arithmetic starts.  (Tried and measured
-    // slower: issuing the next trip's loads before this trip's arithmetic + L2 prefetch of the trip after, at 128 threads x
-    // 5 blocks: 0.184 ms per launch against 0.166 ms; the loop is bound by load latency at 24 warps/SM, not by the FP64 pipe.)
+    // two cells per trip, staged through thread-private shared-memory slots with cp.async, two trips deep: the loads of the
+    // next trip are in flight while this trip's arithmetic runs and cost no registers (ncu of the plain loop: 40 % of the
+    // issue cycles on the long scoreboard at 24 warps/SM; register double-buffering at 5 x 128 threads was slower still)
+    __shared__ R stg[2][8][PRIM_THREADS];
+    auto fetch = [&](int buf, long long cc) {
+        const long long q1 = pad_index(cc, a.nx, a.nxp), q2 = pad_index(cc + stride, a.nx, a.nxp);
+        const R* src[8] = {U0 + q1, U1 + q1, U2 + q1, U3 + q1, U0 + q2, U1 + q2, U2 + q2, U3 + q2};
+#pragma unroll
+        for (int v = 0; v < 8; ++v) {
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(&stg[buf][v][threadIdx.x]);
+            if (sizeof(R) == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src[v]) : "memory");
+            else asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src[v]) : "memory");
+        }
+    };
     long long c = a.c0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    for (; c + stride < a.N; c += 2 * stride) {
-        const long long p1 = pad_index(c, a.nx, a.nxp), p2 = pad_index(c + stride, a.nx, a.nxp);
-        const R E = U0[p1], Mx = U1[p1], My = U2[p1], Mz = U3[p1];
-        const R E2 = U0[p2], Mx2 = U1[p2], My2 = U2[p2], Mz2 = U3[p2];
-        cell(p1, c, E, Mx, My, Mz);
-        cell(p2, c + stride, E2, Mx2, My2, Mz2);
+    int buf = 0;
+    if (c + stride < a.N) fetch(0, c);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    for (; c + stride < a.N; c += 2 * stride, buf ^= 1) {
+        const long long cn = c + 2 * stride;
+        if (cn + stride < a.N) fetch(buf ^ 1, cn);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("cp.async.wait_group 1;" ::: "memory");                  // this trip's eight values have landed
+        const R E = stg[buf][0][threadIdx.x], Mx = stg[buf][1][threadIdx.x], My = stg[buf][2][threadIdx.x],
+                Mz = stg[buf][3][threadIdx.x];
+        const R E2 = stg[buf][4][threadIdx.x], Mx2 = stg[buf][5][threadIdx.x], My2 = stg[buf][6][threadIdx.x],
+                Mz2 = stg[buf][7][threadIdx.x];
+        cell(pad_index(c, a.nx, a.nxp), c, E, Mx, My, Mz);
+        cell(pad_index(c + stride, a.nx, a.nxp), c + stride, E2, Mx2, My2, Mz2);
     }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
     if (c < a.N) {
         const long long p1 = pad_index(c, a.nx, a.nxp);
         cell(p1, c, U0[p1], U1[p1], U2[p1], U3[p1]);
