@@ -43,6 +43,10 @@ struct hydro {
     bool prims_valid;
     // ring sweeps: tensor maps per buffer (0..2 state copies, 3 = L) and direction, march cells per block
     CUtensorMap mapB[4][3], mapW[3], mapP[3];
+    // nf = 5 in fp64 without the limiter: fields 0..3 by the 4-warp kernel (boxes of 4 of the 5 fields) + the baryon
+    // density by the one-warp kernel (boxes of 1 field)
+    CUtensorMap mapB4[4][3], mapB1[4][3], vmapB4[4][3], vmapB1[4][3];
+    bool split5;                        // HYDRO_NO_SPLIT5=1 keeps the 5-warp kernel
     // z-slab decomposition: the same maps over the OWNED planes only (x/y sweeps of the owned planes while the halos are
     // still in flight; output clipping of the z sweep); built by hydro_set_slab
     CUtensorMap vmapB[4][3], vmapW[3], vmapP[3];
@@ -173,13 +177,16 @@ int launch_ring_nf(hydro* h, const void* Us, int slot, int out_b, int un_b, doub
         const int b = buf_index(h, Us);
         if (b < 0 || b > 2 || out_b < 0 || out_b > 3 || un_b > 2) return HYDRO_ESTATE;
         const bool vw = h->view && DIR != 2;                               // everything through the owned-planes view
+        // which box the maps carry: all nf fields, or (5-field state split over two kernels) 4 fields / 1 field
+        CUtensorMap (*mB)[3] = NF == h->nf ? h->mapB : NF == 4 ? h->mapB4 : h->mapB1;
+        CUtensorMap (*vB)[3] = NF == h->nf ? h->vmapB : NF == 4 ? h->vmapB4 : h->vmapB1;
         RingMaps m;
-        m.U = vw ? h->vmapB[b][DIR] : h->mapB[b][DIR];
+        m.U = vw ? vB[b][DIR] : mB[b][DIR];
         m.W = vw ? h->vmapW[DIR] : h->mapW[DIR];
         m.P = vw ? h->vmapP[DIR] : h->mapP[DIR];
-        m.Out = vw ? h->vmapB[out_b][DIR] : h->mapB[out_b][DIR];
-        m.Un = un_b >= 0 ? (vw ? h->vmapB[un_b][DIR] : h->mapB[un_b][DIR]) : m.Out;
-        m.UL = vw ? h->vmapB[3][DIR] : h->mapB[3][DIR];
+        m.Out = vw ? vB[out_b][DIR] : mB[out_b][DIR];
+        m.Un = un_b >= 0 ? (vw ? vB[un_b][DIR] : mB[un_b][DIR]) : m.Out;
+        m.UL = vw ? vB[3][DIR] : mB[3][DIR];
         const int nz_k = vw ? h->own_hi - h->own_lo : h->nz;              // planes the kernel sees
         RingArgs a;
         a.diag = h->diag; a.slot = slot; a.nx = h->nx; a.ny = h->ny; a.nz = nz_k; a.seg_len = h->seg_len[DIR];
@@ -223,6 +230,15 @@ int launch_ring_nf(hydro* h, const void* Us, int slot, int out_b, int un_b, doub
 
 template <typename R, int LIM, int DIR, int OUT>
 int launch_ring_lim(hydro* h, const void* Us, int slot, int out_b, int un_b, double coef, double rk_a, double rk_b) {
+    if constexpr (!LIM && sizeof(R) == 8) {
+        if (h->nf == 5 && h->split5) {
+            int rc = h->order == 5 ? launch_ring_nf<R, 5, 0, DIR, OUT, 4>(h, Us, slot, out_b, un_b, coef, rk_a, rk_b)
+                                   : launch_ring_nf<R, 7, 0, DIR, OUT, 4>(h, Us, slot, out_b, un_b, coef, rk_a, rk_b);
+            if (rc != HYDRO_OK) return rc;
+            return h->order == 5 ? launch_ring_nf<R, 5, 0, DIR, OUT, 1>(h, Us, slot, out_b, un_b, coef, rk_a, rk_b)
+                                 : launch_ring_nf<R, 7, 0, DIR, OUT, 1>(h, Us, slot, out_b, un_b, coef, rk_a, rk_b);
+        }
+    }
     if (h->order == 5)
         return h->nf == 4 ? launch_ring_nf<R, 5, LIM, DIR, OUT, 4>(h, Us, slot, out_b, un_b, coef, rk_a, rk_b)
                           : launch_ring_nf<R, 5, LIM, DIR, OUT, 5>(h, Us, slot, out_b, un_b, coef, rk_a, rk_b);
@@ -243,6 +259,13 @@ int set_smem_attr() {
                                      ring_smem_bytes(NF, OUT, sizeof(R), LIM)) == cudaSuccess ? 0 : 1) +
                (cudaFuncSetAttribute(k_sweep_ring<R, 5, LIM, DIR, OUT, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      ring_smem_bytes(NF, OUT, sizeof(R), LIM)) == cudaSuccess ? 0 : 1);
+}
+template <typename R>
+int set_smem_attrs_baryon() {
+    if constexpr (sizeof(R) != 8) return 0;
+    else return set_smem_attr<R, 0, 0, OUT_STORE, 1>() + set_smem_attr<R, 0, 0, OUT_COMBINE1, 1>() +
+                set_smem_attr<R, 0, 0, OUT_COMBINE, 1>() + set_smem_attr<R, 0, 1, OUT_REDUCE, 1>() +
+                set_smem_attr<R, 0, 2, OUT_REDUCE, 1>();
 }
 template <typename R, int NF>
 int set_smem_attrs() {
@@ -287,26 +310,37 @@ int make_map(hydro* h, CUtensorMap* out, void* base0, int nfb, const unsigned bo
     return HYDRO_OK;
 }
 
-// tensor maps of the planes [k0, k1) of every buffer, per direction
-int build_maps(hydro* h, CUtensorMap mB[4][3], CUtensorMap mW[3], CUtensorMap mP[3], int k0, int k1) {
-    const unsigned NF = (unsigned)h->nf;
-    const unsigned boxes[3][4] = {{RING_CH, 32, 1, NF}, {32, RING_CH, 1, NF}, {32, 1, RING_CH, NF}};
+// tensor maps of the planes [k0, k1) of every buffer, per direction; boxes of `boxf` fields (mW, mP may be null)
+int build_maps(hydro* h, CUtensorMap mB[4][3], CUtensorMap mW[3], CUtensorMap mP[3], int k0, int k1, unsigned boxf) {
+    const unsigned boxes[3][4] = {{RING_CH, 32, 1, boxf}, {32, RING_CH, 1, boxf}, {32, 1, RING_CH, boxf}};
     int rc;
     for (int d = 0; d < 3; ++d) {
         unsigned b1[4] = {boxes[d][0], boxes[d][1], boxes[d][2], 1};
         for (int b = 0; b < 4; ++b)
             if ((rc = make_map(h, &mB[b][d], b < 3 ? h->buf[b] : h->L, h->nf, boxes[d], d == 0, k0, k1)) != HYDRO_OK) return rc;
-        if ((rc = make_map(h, &mW[d], h->W, 1, b1, d == 0, k0, k1)) != HYDRO_OK) return rc;
-        if ((rc = make_map(h, &mP[d], h->P, 1, b1, d == 0, k0, k1)) != HYDRO_OK) return rc;
+        if (mW && (rc = make_map(h, &mW[d], h->W, 1, b1, d == 0, k0, k1)) != HYDRO_OK) return rc;
+        if (mP && (rc = make_map(h, &mP[d], h->P, 1, b1, d == 0, k0, k1)) != HYDRO_OK) return rc;
+    }
+    return HYDRO_OK;
+}
+// all map sets of the planes [k0, k1): full boxes, and the 4 + 1 split of a 5-field state
+int build_map_sets(hydro* h, bool view, int k0, int k1) {
+    int rc;
+    if ((rc = build_maps(h, view ? h->vmapB : h->mapB, view ? h->vmapW : h->mapW, view ? h->vmapP : h->mapP, k0, k1,
+                         (unsigned)h->nf)) != HYDRO_OK) return rc;
+    if (h->nf == 5) {
+        if ((rc = build_maps(h, view ? h->vmapB4 : h->mapB4, 0, 0, k0, k1, 4)) != HYDRO_OK) return rc;
+        if ((rc = build_maps(h, view ? h->vmapB1 : h->mapB1, 0, 0, k0, k1, 1)) != HYDRO_OK) return rc;
     }
     return HYDRO_OK;
 }
 
 int setup_tma(hydro* h) {
     int rc;
-    if ((rc = build_maps(h, h->mapB, h->mapW, h->mapP, 0, h->nz)) != HYDRO_OK) return rc;
-    if ((rc = build_maps(h, h->vmapB, h->vmapW, h->vmapP, 0, h->nz)) != HYDRO_OK) return rc;
-    const int bad = h->prec == 64 ? (h->nf == 4 ? set_smem_attrs<double, 4>() : set_smem_attrs<double, 5>())
+    if ((rc = build_map_sets(h, false, 0, h->nz)) != HYDRO_OK) return rc;
+    if ((rc = build_map_sets(h, true, 0, h->nz)) != HYDRO_OK) return rc;
+    const int bad = h->prec == 64 ? (h->nf == 4 ? set_smem_attrs<double, 4>()
+                                                : set_smem_attrs<double, 5>() + set_smem_attrs<double, 4>() + set_smem_attrs_baryon<double>())
                                   : (h->nf == 4 ? set_smem_attrs<float, 4>() : set_smem_attrs<float, 5>());
     if (bad) {
         h->cuda_err = "cudaFuncSetAttribute(max dynamic shared memory) failed";
@@ -609,6 +643,7 @@ int hydro_create(hydro_t** out, int nx, int ny, int nz, double dx, double dt, co
     h->sigma = 0.0;
     h->limiter = 0;
     { const char* ts = getenv("HYDRO_NO_TAIL_SPLIT"); h->tail_split = !(ts && ts[0] == '1'); }
+    { const char* ts = getenv("HYDRO_NO_SPLIT5"); h->split5 = !(ts && ts[0] == '1'); }
     h->nz_global = nz; h->k_offset = 0; h->own_lo = 0; h->own_hi = nz;
     h->dx = dx; h->dt = dt;
     h->weno_eps = o.weno_eps > 0 ? o.weno_eps : 1e-6;
@@ -732,7 +767,7 @@ int hydro_set_slab(hydro_t* h, int nz_global, int k_offset, int own_lo, int own_
     h->nz_global = nz_global; h->k_offset = k_offset; h->own_lo = own_lo; h->own_hi = own_hi;
     h->prims_valid = false;
     drop_graph(h);
-    return build_maps(h, h->vmapB, h->vmapW, h->vmapP, own_lo, own_hi);
+    return build_map_sets(h, true, own_lo, own_hi);
 }
 
 int hydro_stage_prims(hydro_t* h, int s) {

@@ -4,7 +4,8 @@
 // eq. 1), a-6 (SSP-RK3 stage combination) and a-7 (outflow ghosts) of SURVEY.md 8(a), organised
 // around the one resource that bounds them, the FP64 pipe:
 //
-//   block   = 32 lanes x NF field-warps.  The lanes are 32 neighbouring grid lines (consecutive x for the y/z
+//   block   = 32 lanes x NF field-warps (NF = 1: the single warp of the baryon-density kernel, see BARYON below).
+//             The lanes are 32 neighbouring grid lines (consecutive x for the y/z
 //             sweeps, consecutive y for the x sweep); warp f reconstructs conserved field f, so the warps of a
 //             block share every input row: U (all fields), W = scale/(E+p) and P.
 //   input   = a ring of RING_NSTAGE shared-memory stages, each CH = 8 march cells x 32 lanes of (U[NF], W, P),
@@ -104,6 +105,7 @@ __host__ __device__ constexpr int ring_smem_bytes(int nf, int out, int esz, int 
 #endif
 // resident blocks per SM the kernels are compiled for (registers: 65536 / (32 NF threads x blocks))
 __host__ __device__ constexpr int ring_blocks_per_sm(int nf, int esz, int out = OUT_COMBINE, int lim = 0) {
+    if (nf == 1) return 8;                                    // baryon kernel: one warp, 24-28 KB of shared memory
     if (lim) return (nf == 4 && (out == OUT_REDUCE || out == OUT_STORE)) ? 3 : 2;   // 72 KB / <= 168 registers, else 2
     // nf = 5 in fp64: 3 blocks (<= 136 registers, 64 KB) except the combine kernel with its U^n tiles (84 KB): 2
     return esz == 8 ? (nf == 4 ? RING_F64_BLOCKS : (out != OUT_COMBINE ? 3 : 2)) : (nf == 4 ? RING_F32_BLOCKS : 4);
@@ -111,6 +113,7 @@ __host__ __device__ constexpr int ring_blocks_per_sm(int nf, int esz, int out = 
 
 struct RingMaps {
     CUtensorMap U, W, P;       // loads: stage state (NF fields per box), W and P (one field per box)
+                               // NF = 1 (baryon kernel): U, Un, Out are one-field-box maps of the 5-field buffers, P is unused
     CUtensorMap Un;            // load : U^n at the output cells (OUT_COMBINE)
     CUtensorMap Out;           // store / reduce target (NF fields per box)
     CUtensorMap UL;            // load : first-order update U^L (limiter, R16)
@@ -508,6 +511,12 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
     uint64_t* full = (uint64_t*)(tht + (LIM ? RING_SUB : 0));
     uint64_t* full_ul = full + RING_NSTAGE;
 
+    // NF = 1: the baryon density N_B (field 4) of a 5-field state on its own, F = N_B v_d: a one-warp block whose stage
+    // holds [N_B][W][M_d] (M_d in the slot P has otherwise).  With the 4-warp kernel on fields 0..3 it replaces the 5-warp
+    // kernel in fp64, whose 160-thread blocks cannot hold the pipelined row loop at 3 blocks/SM.
+    constexpr bool BARYON = (NF == 1);
+    constexpr int F0 = BARYON ? 4 : 0;                                 // first field of the boxes
+    static_assert(!(BARYON && LIM), "the limiter needs all energy-momentum fields in one block");
     const int lane = threadIdx.x, f = threadIdx.y;
     const bool leader = (lane == 0 && f == 0);
     const int nd = DIR == 0 ? a.nx : DIR == 1 ? a.ny : a.nz;
@@ -558,12 +567,13 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
         coords(s0 - 4 + m * RING_CH, c0, c1, c2);
         const bool with_un = (OUT == OUT_COMBINE) && m > 0;
         mbar_expect_tx(&full[st], STAGE_BYTES + (with_un ? UN_BYTES : 0u));
-        tma_load_4d(dst, &maps.U, &full[st], c0, c1, c2, 0);
+        tma_load_4d(dst, &maps.U, &full[st], c0, c1, c2, F0);
         tma_load_4d(dst + NF * RING_SUB, &maps.W, &full[st], c0, c1, c2, 0);
-        tma_load_4d(dst + (NF + 1) * RING_SUB, &maps.P, &full[st], c0, c1, c2, 0);
+        if (BARYON) tma_load_4d(dst + (NF + 1) * RING_SUB, &maps.U, &full[st], c0, c1, c2, 1 + DIR);
+        else tma_load_4d(dst + (NF + 1) * RING_SUB, &maps.P, &full[st], c0, c1, c2, 0);
         if (with_un) {
             coords(s0 + (m - 1) * RING_CH, c0, c1, c2);                // the cells chunk m emits
-            tma_load_4d(unt + (m & 1) * NF * RING_SUB, &maps.Un, &full[st], c0, c1, c2, 0);
+            tma_load_4d(unt + (m & 1) * NF * RING_SUB, &maps.Un, &full[st], c0, c1, c2, F0);
         }
     };
     auto issue_ul = [&](int m) {                                       // leader only (limiter): U^L of chunk m's cells
@@ -576,8 +586,8 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
         int c0, c1, c2;
         coords(s0 + (m - 1) * RING_CH, c0, c1, c2);
         const R* src = outt + (m & 1) * NF * RING_SUB;
-        if (OUT == OUT_REDUCE) tma_reduce_add_4d(&maps.Out, src, c0, c1, c2, 0);
-        else tma_store_4d(&maps.Out, src, c0, c1, c2, 0);
+        if (OUT == OUT_REDUCE) tma_reduce_add_4d(&maps.Out, src, c0, c1, c2, F0);
+        else tma_store_4d(&maps.Out, src, c0, c1, c2, F0);
         tma_commit();
     };
     if (leader) {
@@ -603,7 +613,7 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
     cx.rk_a = (R)a.rk_a;
     cx.rk_b = (R)a.rk_b;
     cx.lane = lane;
-    const bool is_energy = (f == 0), is_normal = (f == 1 + DIR);
+    const bool is_energy = !BARYON && f == 0, is_normal = !BARYON && f == 1 + DIR;
     cx.kE = is_energy ? R(1) : R(0);
 
     for (int m = 0; m < nchunks; ++m) {
@@ -641,7 +651,7 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
         }
 
         cx.pu.set(st + f * RING_SUB, lane);
-        cx.pmd.set(st + (1 + DIR) * RING_SUB, lane);
+        cx.pmd.set(st + (BARYON ? NF + 1 : 1 + DIR) * RING_SUB, lane);
         cx.pa.set(is_energy ? st + (1 + DIR) * RING_SUB : st + f * RING_SUB, lane);
         cx.pw.set(is_energy ? zeros : st + NF * RING_SUB, lane);
         cx.pp.set(is_normal ? st + (NF + 1) * RING_SUB : zeros, lane);
