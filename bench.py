@@ -56,15 +56,35 @@ def variant_key(cfg, precision, order, nf, limiter):
 
 
 def ncu_rows(variant):
-    """{kernel class: row dict} of the committed ncu summary for this variant ({} if none)."""
+    """{kernel class: [row dicts]} of the committed ncu summary for this variant ({} if none).  A class has several rows
+    when its passes were captured in several instantiations (x: COMBINE1 of stage 1 and COMBINE of stages 2, 3; 5-field
+    states: the 4-field and the 1-field kernel of every pass)."""
     import csv
     out = {}
     if os.path.exists(NCU_TABLE):
         with open(NCU_TABLE) as f:
             for row in csv.DictReader(l for l in f if not l.startswith("#")):
                 if row["variant"] == variant:
-                    out[row["kernel"]] = row
+                    out.setdefault(row["kernel"], []).append(row)
     return out
+
+
+def ncu_pass_mean(rows, key):
+    """Mean over the nine directional passes of a step of an ncu counter: per direction, the kernels of one pass add up
+    (nf4 + nf1 instantiations), and the x direction is COMBINE1 once and COMBINE twice per step."""
+    tot, n = 0.0, 0
+    for cls in ("sweep_x", "sweep_y", "sweep_z"):
+        by_out = {}
+        for r in rows.get(cls, []):
+            by_out.setdefault(r["template"].split(";")[3], []).append(float(r[key]))
+        if not by_out:
+            return None
+        if cls == "sweep_x" and "COMBINE1" in by_out and "COMBINE" in by_out:
+            tot += sum(by_out["COMBINE1"]) + 2.0 * sum(by_out["COMBINE"])
+        else:
+            tot += 3.0 * sum(next(iter(by_out.values())))
+        n += 3
+    return tot / n
 
 
 def max_over_ranks(values, world, device):
@@ -373,29 +393,33 @@ def main():
         # dominant kernel class: the WENO7-LF sweep kernels; flops per launch = (sweep flops per cell per stage / 3) * cells
         fl_sweeps = (FLOPS_SWEEPS_STAGE if args.weno_order == 7 else FLOPS_SWEEPS_STAGE_W5)[nf]
         fl_stage = (FLOPS_STAGE if args.weno_order == 7 else FLOPS_STAGE_W5)[nf]
+        # one "launch" of the dominant kernel class = one directional pass over the grid (9 per RK3 step).  A 5-field fp64
+        # state is swept by two kernels per pass (fields 0..3 + the baryon density): their times add up.
+        passes = 9.0 * args.steps
         fl_launch = fl_sweeps / 3.0 * cells
-        achieved = fl_launch / (sw_ms / sw_n * 1e-3) / 1e12 if sw_n else 0.0
+        achieved = fl_launch / (sw_ms / passes * 1e-3) / 1e12 if sw_n else 0.0
         nominal = FP64_NOMINAL_TF * (1 if args.precision == 64 else 2)
         esz = args.precision // 8
-        sweeps_per_step = sw_n / args.steps if sw_n else 9.0
+        sweeps_per_step = 9.0
         rows = ncu_rows(variant_key(cfg, args.precision, args.weno_order, nf, args.limiter))
         from paper_1511_02137_b200 import build as B
         sha = B.source_sha()
-        srows = [rows[k] for k in ("sweep_x", "sweep_y", "sweep_z") if k in rows]
+        srows = [r for k in ("sweep_x", "sweep_y", "sweep_z") for r in rows.get(k, [])]
         traffic = inst64 = pipe = None
-        if srows:
-            # per launch, mean over the step's sweep launches: stage 1's x kernel (COMBINE1) reads no U^n and is listed
-            # separately when it was captured
-            traffic = sum(float(r["dram_read_B"]) + float(r["dram_write_B"]) for r in srows) / len(srows)
-            inst64 = sum(float(r["inst_fp64"]) for r in srows) / len(srows)
-            pipe = sum(float(r["pipe_fp64_pct"]) for r in srows) / len(srows) / 100.0
-        avg_s = sw_ms / sw_n * 1e-3 if sw_n else None
+        if srows and ncu_pass_mean(rows, "dram_read_B") is not None:
+            traffic = ncu_pass_mean(rows, "dram_read_B") + ncu_pass_mean(rows, "dram_write_B")
+            inst64 = ncu_pass_mean(rows, "inst_fp64")
+            pipe = sum(float(r["pipe_fp64_pct"]) * float(r["duration_us"]) for r in srows) / \
+                sum(float(r["duration_us"]) for r in srows) / 100.0
+        avg_s = sw_ms / passes * 1e-3 if sw_n else None
+        kernels_per_pass = sw_n / passes if sw_n else 1.0
         roof = {"bound": "alu", "kernel": "k_sweep_ring<x|y|z> (WENO%d-LF flux + divergence + RK3 combine)" % args.weno_order,
                 "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf,
                 "peak_kind": "measured in this run: register-resident %s chain on all SMs (hydro_measure_alu_peak)" %
                              ("DFMA" if args.precision == 64 else "FFMA"),
                 "peak_nominal": nominal, "frac_of_nominal": achieved / nominal,
-                "flops_per_launch": fl_launch, "avg_launch_ms": sw_ms / sw_n if sw_n else None,
+                "flops_per_launch": fl_launch, "avg_launch_ms": sw_ms / passes if sw_n else None,
+                "kernels_per_launch": kernels_per_pass,
                 "share_of_step": sw_ms / all_ms if all_ms else None,
                 "kernel_ms_per_step": {k: v["ms"] / args.steps for k, v in kt.items()},
                 "ms_per_step_profiled_pass": ms_profiled / args.steps,
@@ -407,7 +431,7 @@ def main():
                 "fp64_pipe_busy_ncu": pipe if args.precision == 64 else None,
                 "traffic": traffic,
                 "traffic_source": "profiles/r2_ncu_kernels.csv (ncu --set full: dram__bytes_read.sum + dram__bytes_write.sum per "
-                                  "launch, mean of the x, y, z sweep kernels)" if srows else None,
+                                  "directional pass, mean over the nine passes of a step)" if srows else None,
                 "profile_csrc_sha": srows[0]["csrc_sha"] if srows else None, "csrc_sha": sha,
                 "profile_stale": (srows[0]["csrc_sha"] != sha) if srows else None,
                 # unique bytes of a fully fused stage, (2 + 3 + 3) x nf x sizeof(real) per cell-update, spread

@@ -358,10 +358,12 @@ __device__ __forceinline__ R theta_cell(const R W0[4], const R a[4], R sgn) {
 
 // theta of the face of chunk row r (between march cells i = cm + r - 4 and i + 1) for this lane: reads the corrections of
 // the four energy-momentum fields from the chunk's output tiles (where phase A left them) and U^L of the two cells from
-// the two U^L tiles (rows r-4, r-3; the previous chunk's tile for negative rows).  Cells outside the grid impose no condition.  Returns 1 if theta < 1.
-template <int r, int DIR, int NF, typename R>
-__device__ __forceinline__ int theta_row(const R* st, const R* stp, const R* xc_all, R* th, int lane, int cm, int nd, R k3lam) {
-    constexpr int ULB = 0;             // st / stp: the U^L tiles of this chunk / of the previous chunk
+// the two U^L tiles (rows r-4, r-3; the previous chunk's tile for negative rows).  Cells outside the grid impose no
+// condition.  Returns 1 if theta < 1.  r is a RUN-TIME argument on purpose: every warp calls this for its two rows, and
+// eight compile-time copies (each with two divisions and two square roots on its slow path) made the limiter kernels
+// instruction-cache bound (ncu r2_d: 40 % of the issue cycles stalled on "no instruction").
+template <int DIR, int NF, typename R>
+__device__ __noinline__ int theta_row(int r, const R* st, const R* stp, const R* xc_all, R* th, int lane, int cm, int nd, R k3lam) {
     const int o = sub_off<DIR, R>(r, lane);
     R a[4];
 #pragma unroll
@@ -369,20 +371,18 @@ __device__ __forceinline__ int theta_row(const R* st, const R* stp, const R* xc_
     const int i = cm + r - 4;
     R theta = R(1);
     if (i >= 0 && i <= nd - 1) {
-        constexpr int rl = (r + 4) & 7;
+        const int rl = (r + 4) & 7;
         const R* s = r < 4 ? stp : st;
         const int ol = sub_off<DIR, R>(rl, lane);
-        const R W0[4] = {s[(ULB + 0) * RING_SUB + ol], s[(ULB + 1) * RING_SUB + ol], s[(ULB + 2) * RING_SUB + ol],
-                         s[(ULB + 3) * RING_SUB + ol]};
+        const R W0[4] = {s[ol], s[RING_SUB + ol], s[2 * RING_SUB + ol], s[3 * RING_SUB + ol]};
         const R t = theta_cell<R>(W0, a, R(-1));
         theta = t < theta ? t : theta;
     }
     if (i + 1 >= 0 && i + 1 <= nd - 1) {
-        constexpr int rr = (r + 5) & 7;
+        const int rr = (r + 5) & 7;
         const R* s = r < 3 ? stp : st;
         const int orr = sub_off<DIR, R>(rr, lane);
-        const R W0[4] = {s[(ULB + 0) * RING_SUB + orr], s[(ULB + 1) * RING_SUB + orr], s[(ULB + 2) * RING_SUB + orr],
-                         s[(ULB + 3) * RING_SUB + orr]};
+        const R W0[4] = {s[orr], s[RING_SUB + orr], s[2 * RING_SUB + orr], s[3 * RING_SUB + orr]};
         const R t = theta_cell<R>(W0, a, R(1));
         theta = t < theta ? t : theta;
     }
@@ -677,7 +677,7 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
                 mbar_wait(&full_ul[m & 1], (m >> 1) & 1);
                 __syncthreads();
                 if (f == 0) {
-                    const int n1 = theta_row<7, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, (R)a.k3lam);
+                    const int n1 = theta_row<DIR, NF, R>(7, ul_cur, ul_prev, xcm, tht, lane, cm, nd, (R)a.k3lam);
                     // inner segment starts are counted by the segment before; z sweep: the face below plane 0
                     if (s0 == 0 && (DIR == 2 ? a.own_lo == 0 : (tfix >= a.own_lo && tfix < a.own_hi))) nlim_local += n1;
                 }
@@ -692,23 +692,17 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
             mbar_wait(&full_ul[m & 1], (m >> 1) & 1);
             __syncthreads();
             const R k3 = (R)a.k3lam;
-            // faces of rows 2f, 2f+1: lower cells cm + 2f - 4, cm + 2f - 3
-            const int il = cm + 2 * f - 4;
-            const bool cnt0 = DIR == 2 ? (il >= a.own_lo && il < a.own_hi) : (tfix >= a.own_lo && tfix < a.own_hi);
-            const bool cnt1 = DIR == 2 ? (il + 1 >= a.own_lo && il + 1 < a.own_hi) : cnt0;
             int n0 = 0, n1 = 0;
-            switch (f) {
-                case 0: n0 = theta_row<0, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3);
-                        n1 = theta_row<1, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3); break;
-                case 1: n0 = theta_row<2, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3);
-                        n1 = theta_row<3, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3); break;
-                case 2: n0 = theta_row<4, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3);
-                        n1 = theta_row<5, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3); break;
-                case 3: n0 = theta_row<6, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3);
-                        n1 = theta_row<7, DIR, NF, R>(ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3); break;
-                default: break;
+            if (f < 4) {                                            // warp f: the faces of rows 2f and 2f + 1
+                n0 = theta_row<DIR, NF, R>(2 * f, ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3);
+                n1 = theta_row<DIR, NF, R>(2 * f + 1, ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3);
             }
-            nlim_local += (cnt0 ? n0 : 0) + (cnt1 ? n1 : 0);
+            if (n0 | n1) {                                          // rare: only now look at ownership (z-slabs)
+                const int il = cm + 2 * f - 4;                      // faces of rows 2f, 2f+1: lower cells il, il + 1
+                const bool cnt0 = DIR == 2 ? (il >= a.own_lo && il < a.own_hi) : (tfix >= a.own_lo && tfix < a.own_hi);
+                const bool cnt1 = DIR == 2 ? (il + 1 >= a.own_lo && il + 1 < a.own_hi) : cnt0;
+                nlim_local += (cnt0 ? n0 : 0) + (cnt1 ? n1 : 0);
+            }
             __syncthreads();
             cx.template emit_lim<0>(); cx.template emit_lim<1>(); cx.template emit_lim<2>(); cx.template emit_lim<3>();
             cx.template emit_lim<4>(); cx.template emit_lim<5>(); cx.template emit_lim<6>(); cx.template emit_lim<7>();
