@@ -62,3 +62,26 @@ def test_reference_arm_non_zero_ranks_do_no_work(monkeypatch, capsys):
     import bench
     bench.run_reference(argparse.Namespace(config=3, steps=1, warmup=0, gpus=2), rank=1)
     assert capsys.readouterr().out == ""
+
+
+def test_ncu_table_is_readable_and_covers_the_headline_variant():
+    """bench.py takes its ncu-only counters (DRAM bytes, FP64 warp-instructions, pipe utilisation) from the committed
+    summary profiles/r2_ncu_kernels.csv: the table must parse, carry the sha of the sources it was taken at, and hold
+    the three sweep classes of the headline variant (config 3, fp64, WENO7, nf = 4) and of the variants with a claim."""
+    sys.path.insert(0, ROOT)
+    import bench
+    for variant in ("cfg3_f64_w7_nf4_lim0", "cfg3_f64_w5_nf4_lim0", "cfg3_f32_w7_nf4_lim0", "cfg3_f64_w7_nf4_lim1",
+                    "cfg4_f64_w7_nf5_lim0"):
+        rows = bench.ncu_rows(variant)
+        assert {"sweep_x", "sweep_y", "sweep_z", "prim"} <= set(rows), variant
+        shas = {r["csrc_sha"] for rs in rows.values() for r in rs}
+        assert len(shas) == 1 and len(next(iter(shas))) == 16
+        traffic = bench.ncu_pass_mean(rows, "dram_read_B") + bench.ncu_pass_mean(rows, "dram_write_B")
+        cells = 512 ** 3 if variant.startswith("cfg4") else 256 ** 3
+        nf, esz = (5 if "nf5" in variant else 4), (4 if "f32" in variant else 8)
+        floor = 8.0 * nf * esz * cells / 9.0                  # SURVEY 8(d): unique bytes of a fused stage, per pass
+        assert 2.0 * floor < traffic < 6.0 * floor, (variant, traffic / floor)
+    # a 5-field fp64 pass is two kernels (fields 0..3 + baryon density): their counters add up per pass
+    rows = bench.ncu_rows("cfg4_f64_w7_nf5_lim0")
+    assert len(rows["sweep_y"]) == 2 and len(rows["sweep_x"]) == 4
+    assert bench.variant_key(3, 64, 7, 4, False) == "cfg3_f64_w7_nf4_lim0"
