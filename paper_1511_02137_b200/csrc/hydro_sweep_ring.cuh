@@ -8,7 +8,7 @@
 //             The lanes are 32 neighbouring grid lines (consecutive x for the y/z
 //             sweeps, consecutive y for the x sweep); warp f reconstructs conserved field f, so the warps of a
 //             block share every input row: U (all fields), W = scale/(E+p) and P.
-//   input   = a ring of RING_NSTAGE shared-memory stages, each CH = 8 march cells x 32 lanes of (U[NF], W, P),
+//   input   = a ring of 2 or 3 (ring_nstage) shared-memory stages, each CH = 8 march cells x 32 lanes of (U[NF], W, P),
 //             filled by one thread with cp.async.bulk.tensor (TMA) box loads that complete on an mbarrier, one
 //             chunk ahead of the arithmetic.  The x sweep uses the 64-byte TMA swizzle so that lane = row reads
 //             its own row with a 2-way bank conflict at most.
@@ -33,10 +33,15 @@
 namespace hydro_dev {
 
 constexpr int RING_CH = 8;                 // march cells per chunk
-constexpr int RING_NSTAGE = 3;             // input ring depth: chunks m-1 (still read), m (current), m+1 (in flight)
+constexpr int RING_NSTAGE_MAX = 3;
 constexpr int RING_SUB = RING_CH * 32;     // reals per sub-tile (one field, one chunk)
 
 enum { OUT_STORE = 0, OUT_REDUCE = 1, OUT_COMBINE1 = 2, OUT_COMBINE = 3 };
+// input ring depth: chunk m (current) and m+1 (in flight); the combine kernels also read U_s of chunk m-1's last rows (their
+// output cells lag the march by 4) -- unless the limiter's U^L tiles replace U_s there
+__host__ __device__ constexpr int ring_nstage(int out, int lim) {
+    return ((out == OUT_COMBINE1 || out == OUT_COMBINE) && !lim) ? 3 : 2;
+}
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -90,10 +95,10 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // shared-memory plan of one launch (host and device agree through these functions); units: reals
 __host__ __device__ constexpr int ring_stage_reals(int nf, int lim = 0) { return (lim ? nf + 2 : nf + 2) * RING_SUB; }
 __host__ __device__ constexpr int ring_smem_bytes(int nf, int out, int esz, int lim = 0) {
-    return (RING_NSTAGE * ring_stage_reals(nf, lim)       // input ring
+    return (ring_nstage(out, lim) * ring_stage_reals(nf, lim)   // input ring
             + (lim ? (2 * nf + 1) * RING_SUB : 0)          // limiter: two U^L tiles (this chunk, previous chunk) + theta tile
             + 2 * nf * RING_SUB                            // two output tiles
-            + (out == OUT_COMBINE ? 2 * nf * RING_SUB : 0) // two U^n tiles
+            + (out == OUT_COMBINE ? (lim ? 1 : 2) * nf * RING_SUB : 0)   // U^n tiles: two riding with the input stages; limiter: one
             + RING_SUB) * esz                              // one tile of zeros
            + 64;                                           // mbarriers
 }
@@ -106,7 +111,7 @@ __host__ __device__ constexpr int ring_smem_bytes(int nf, int out, int esz, int 
 // resident blocks per SM the kernels are compiled for (registers: 65536 / (32 NF threads x blocks))
 __host__ __device__ constexpr int ring_blocks_per_sm(int nf, int esz, int out = OUT_COMBINE, int lim = 0) {
     if (nf == 1) return 8;                                    // baryon kernel: one warp, 24-28 KB of shared memory
-    if (lim) return (nf == 4 && (out == OUT_REDUCE || out == OUT_STORE)) ? 3 : 2;   // 72 KB / <= 168 registers, else 2
+    if (lim) return nf == 4 ? 3 : 2;                          // <= 68 KB and <= 168 registers; 5 warps: 2
     // nf = 5 in fp64: 3 blocks (<= 136 registers, 64 KB) except the combine kernel with its U^n tiles (84 KB): 2
     return esz == 8 ? (nf == 4 ? RING_F64_BLOCKS : (out != OUT_COMBINE ? 3 : 2)) : (nf == 4 ? RING_F32_BLOCKS : 4);
 }
@@ -503,13 +508,15 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
     constexpr uint32_t STAGE_BYTES = STAGE_REALS * sizeof(R);
     constexpr uint32_t UN_BYTES = NF * RING_SUB * sizeof(R);
     R* stages = (R*)smem;
-    R* outt = stages + RING_NSTAGE * STAGE_REALS;                      // two output tiles of NF sub-tiles
-    R* unt = outt + 2 * NF * RING_SUB;                                 // OUT_COMBINE: two U^n tiles
-    R* zeros = unt + (OUT == OUT_COMBINE ? 2 * NF * RING_SUB : 0);
+    constexpr int NSTAGE = ring_nstage(OUT, LIM);
+    R* outt = stages + NSTAGE * STAGE_REALS;                           // two output tiles of NF sub-tiles
+    R* unt = outt + 2 * NF * RING_SUB;                                 // OUT_COMBINE: two U^n tiles (limiter: one)
+    R* zeros = unt + (OUT == OUT_COMBINE ? (LIM ? 1 : 2) * NF * RING_SUB : 0);
     R* ult = zeros + RING_SUB;                                         // limiter: two U^L tiles of NF sub-tiles, then the theta tile
     R* tht = ult + (LIM ? 2 * NF * RING_SUB : 0);
     uint64_t* full = (uint64_t*)(tht + (LIM ? RING_SUB : 0));
-    uint64_t* full_ul = full + RING_NSTAGE;
+    uint64_t* full_ul = full + RING_NSTAGE_MAX;
+    uint64_t* full_un = full_ul + 2;                                   // limiter + OUT_COMBINE: the single U^n tile
 
     // NF = 1: the baryon density N_B (field 4) of a 5-field state on its own, F = N_B v_d: a one-warp block whose stage
     // holds [N_B][W][M_d] (M_d in the slot P has otherwise).  With the 4-warp kernel on fields 0..3 it replaces the 5-warp
@@ -548,8 +555,8 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
 
     if (leader) {
 #pragma unroll
-        for (int s = 0; s < RING_NSTAGE; ++s) mbar_init(&full[s], 1);
-        if (LIM) { mbar_init(&full_ul[0], 1); mbar_init(&full_ul[1], 1); }
+        for (int s = 0; s < NSTAGE; ++s) mbar_init(&full[s], 1);
+        if (LIM) { mbar_init(&full_ul[0], 1); mbar_init(&full_ul[1], 1); mbar_init(full_un, 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int i = f * 32 + lane; i < RING_SUB; i += 32 * NF) zeros[i] = R(0);
@@ -561,11 +568,11 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
         else { c0 = t0; c1 = tfix; c2 = cm; }
     };
     auto issue = [&](int m) {                                          // leader only
-        const int st = m % RING_NSTAGE;
+        const int st = m % NSTAGE;
         R* dst = stages + st * STAGE_REALS;
         int c0, c1, c2;
         coords(s0 - 4 + m * RING_CH, c0, c1, c2);
-        const bool with_un = (OUT == OUT_COMBINE) && m > 0;
+        const bool with_un = (OUT == OUT_COMBINE) && !LIM && m > 0;
         mbar_expect_tx(&full[st], STAGE_BYTES + (with_un ? UN_BYTES : 0u));
         tma_load_4d(dst, &maps.U, &full[st], c0, c1, c2, F0);
         tma_load_4d(dst + NF * RING_SUB, &maps.W, &full[st], c0, c1, c2, 0);
@@ -581,6 +588,14 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
         coords(s0 - 4 + m * RING_CH, c0, c1, c2);
         mbar_expect_tx(&full_ul[m & 1], UN_BYTES);
         tma_load_4d(ult + (m & 1) * NF * RING_SUB, &maps.UL, &full_ul[m & 1], c0, c1, c2, 0);
+    };
+    // limiter + OUT_COMBINE: U^n of the cells chunk m emits into the one U^n tile, issued at the top of chunk m (phase C of
+    // chunk m-1 was its last reader) and needed only in phase C, a whole phase A later
+    auto issue_un = [&](int m) {                                       // leader only
+        int c0, c1, c2;
+        coords(s0 + (m - 1) * RING_CH, c0, c1, c2);
+        mbar_expect_tx(full_un, UN_BYTES);
+        tma_load_4d(unt, &maps.Un, full_un, c0, c1, c2, F0);
     };
     auto flush = [&](int m) {                                          // leader only: write back chunk m's outputs
         int c0, c1, c2;
@@ -624,13 +639,16 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
             __syncthreads();                                           // everyone is done with chunk m-1
             if (leader) {
                 if (m > 1) flush(m - 1);
-                if (m + 1 < nchunks) issue(m + 1);                     // overwrites chunk m-2
+                if (m + 1 < nchunks) issue(m + 1);                     // overwrites chunk m+1-NSTAGE
                 if (LIM) issue_ul(m);                                  // overwrites chunk m-2's U^L (phase B of m-1 is over)
+                if (LIM && OUT == OUT_COMBINE) issue_un(m);
             }
         }
-        R* st = stages + (m % RING_NSTAGE) * STAGE_REALS;
-        const R* stp = stages + ((m + RING_NSTAGE - 1) % RING_NSTAGE) * STAGE_REALS;   // chunk m-1
-        mbar_wait(&full[m % RING_NSTAGE], (m / RING_NSTAGE) & 1);
+        R* st = stages + (m % NSTAGE) * STAGE_REALS;
+        // chunk m-1; with two stages it is chunk m+1's target, but the only reader outside the 3-stage combine kernels is
+        // the ghost fix-up of a line's LAST chunk, after which nothing is loaded
+        const R* stp = stages + ((m + NSTAGE - 1) % NSTAGE) * STAGE_REALS;
+        mbar_wait(&full[m % NSTAGE], (m / NSTAGE) & 1);
 
         // a-7: ghost rows (block-uniform test; at most the first and the last two chunks of a grid line)
         if (cm < 0 || cm + RING_CH - 1 > nd - 1) {
@@ -659,7 +677,7 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
             cx.pus[0].set(LIM ? ult + ((m + 1) & 1) * NF * RING_SUB + f * RING_SUB : stp + f * RING_SUB, lane);
             cx.pus[1].set(LIM ? ult + (m & 1) * NF * RING_SUB + f * RING_SUB : st + f * RING_SUB, lane);
         }
-        if (OUT == OUT_COMBINE) cx.pun.set(unt + (m & 1) * NF * RING_SUB + f * RING_SUB, lane);
+        if (OUT == OUT_COMBINE) cx.pun.set(unt + (LIM ? 0 : (m & 1)) * NF * RING_SUB + f * RING_SUB, lane);
         cx.out = outt + (m & 1) * NF * RING_SUB + f * RING_SUB;
 
         const R* ul_cur = ult + (m & 1) * NF * RING_SUB;            // limiter: U^L tiles of this / the previous chunk
@@ -703,6 +721,7 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
                 const bool cnt1 = DIR == 2 ? (il + 1 >= a.own_lo && il + 1 < a.own_hi) : cnt0;
                 nlim_local += (cnt0 ? n0 : 0) + (cnt1 ? n1 : 0);
             }
+            if (OUT == OUT_COMBINE) mbar_wait(full_un, (m - 1) & 1);
             __syncthreads();
             cx.template emit_lim<0>(); cx.template emit_lim<1>(); cx.template emit_lim<2>(); cx.template emit_lim<3>();
             cx.template emit_lim<4>(); cx.template emit_lim<5>(); cx.template emit_lim<6>(); cx.template emit_lim<7>();

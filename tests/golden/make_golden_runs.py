@@ -14,6 +14,10 @@ Cases (name: config, steps, oracle options):
     cfg3          BASELINE config 3, 256^3, 120 steps                    (the graded benchmark)
     cfg3_fp32     config 3 with the fp32 variant's reading R10: initial state rounded to fp32, delta = 1e-5
     cfg3_lim      config 3 with the positivity-preserving flux limiter (reading R16)
+    cfg3_w5       config 3 with the WENO5 variant, 120 steps
+    cfg4_s6       BASELINE config 4 at FULL SIZE (512^3, nf = 5, two jets), the first 6 of its 200 steps (the whole run is
+                  ~4 h of oracle time; 6 steps are ~10 min and ~40 GB) -- the one oracle comparison at the size where the
+                  nf = 5 kernels run several waves with tail splitting
 
 What is stored per case (numpy .npz):
     idx      (ncells, 3) int32   (k, j, i) of the sampled cells: every 8th cell per axis (offset 3), the full-resolution
@@ -42,13 +46,15 @@ CASES = {
     "cfg3": dict(config=3, delta=1e-10, fp32_input=False, limiter=False),
     "cfg3_fp32": dict(config=3, delta=1e-5, fp32_input=True, limiter=False),
     "cfg3_lim": dict(config=3, delta=1e-10, fp32_input=False, limiter=True),
+    "cfg3_w5": dict(config=3, delta=1e-10, fp32_input=False, limiter=False, weno_order=5),
+    "cfg4_s6": dict(config=4, delta=1e-10, fp32_input=False, limiter=False, steps=6),
 }
 
 
-def sample_indices(c):
+def sample_indices(c, steps):
     """(k, j, i) of the stored cells (docstring above).  Integer work on the config's jet geometry (R6, R7)."""
     nx, ny, nz = c["n"]
-    dx, dt, steps = c["dx"], c["dt"], c["steps"]
+    dx, dt = c["dx"], c["dt"]
     keep = np.zeros((nz, ny, nx), bool)
     keep[3::8, 3::8, 3::8] = True
     for pos, d in c["jets"]:
@@ -67,30 +73,34 @@ def sample_indices(c):
 def run_case(name):
     case = CASES[name]
     c = S.CONFIGS[case["config"]]
+    steps = case.get("steps", c["steps"])
     U0 = S.make_state(case["config"])
     if case["fp32_input"]:
         U0 = U0.astype(np.float32).astype(np.float64)
-    o = O.Oracle(*c["n"], c["dx"], c["dt"], nfields=c["nf"], v_cap_delta=case["delta"])
+    o = O.Oracle(*c["n"], c["dx"], c["dt"], nfields=c["nf"], v_cap_delta=case["delta"],
+                 weno_order=case.get("weno_order", 7))
     o.set_state(U0)
     for pos, d in c["jets"]:
         o.add_jet(pos, d, S.KAPPA_RAD, S.KAPPA_COLL, S.CR_OVER_CF)
     o.set_limiter(case["limiter"])
+    del U0
     t0 = time.time()
-    for s in range(c["steps"]):
+    for s in range(steps):
         o.step(1)
-        if (s + 1) % 10 == 0:
-            print("%s: step %d / %d, %.0f s" % (name, s + 1, c["steps"], time.time() - t0), flush=True)
+        if (s + 1) % 10 == 0 or steps < 10:
+            print("%s: step %d / %d, %.0f s" % (name, s + 1, steps, time.time() - t0), flush=True)
     U = o.get_fields(0)
     dg = o.diag()
-    assert dg["has_nan"] == 0 and dg["step"] == c["steps"]
-    idx = sample_indices(c)
+    assert dg["has_nan"] == 0 and dg["step"] == steps
+    idx = sample_indices(c, steps)
     out = os.path.join(HERE, "run_%s.npz" % name)
     np.savez(out, idx=idx, U=U[:, idx[:, 0], idx[:, 1], idx[:, 2]],
              fmax=np.abs(U).max(axis=(1, 2, 3)), fsum=U.sum(axis=(1, 2, 3), dtype=np.longdouble).astype(np.float64),
              fabs=np.abs(U).sum(axis=(1, 2, 3), dtype=np.longdouble).astype(np.float64),
              alpha=dg["alpha"], deposited=dg["deposited"], ncap=np.int64(dg["ncap"]), nlim=np.int64(o.limited_faces()),
              step=np.int64(dg["step"]), delta=case["delta"], limiter=np.int64(case["limiter"]),
-             config=np.int64(case["config"]), steps=np.int64(c["steps"]), fp32_input=np.int64(case["fp32_input"]))
+             config=np.int64(case["config"]), steps=np.int64(steps), fp32_input=np.int64(case["fp32_input"]),
+             weno_order=np.int64(case.get("weno_order", 7)))
     print("%s: wrote %s (%d cells, %.1f MB), ncap %d, nlim %d, %.0f s" %
           (name, out, len(idx), os.path.getsize(out) / 1e6, dg["ncap"], o.limited_faces(), time.time() - t0), flush=True)
     o.close()
