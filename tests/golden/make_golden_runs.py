@@ -20,7 +20,7 @@ Cases (name: config, steps, oracle options):
                   nf = 5 kernels run several waves with tail splitting
 
 What is stored per case (numpy .npz):
-    idx      (ncells, 3) int32   (k, j, i) of the sampled cells: every 8th cell per axis (offset 3), the full-resolution
+    idx      (ncells, 3) int32   (k, j, i) of the sampled cells: every 8th cell per axis (offset 3; cfg4_s6: every 16th), the full-resolution
                                  line j = ny/2, k = nz/2 (the jet line y = z = 0+, R7) and the box of +-8 cells around
                                  the jet's track (all cells the jet deposits into during the run)
     U        (nf, ncells) f64    final conserved state at those cells
@@ -47,16 +47,16 @@ CASES = {
     "cfg3_fp32": dict(config=3, delta=1e-5, fp32_input=True, limiter=False),
     "cfg3_lim": dict(config=3, delta=1e-10, fp32_input=False, limiter=True),
     "cfg3_w5": dict(config=3, delta=1e-10, fp32_input=False, limiter=False, weno_order=5),
-    "cfg4_s6": dict(config=4, delta=1e-10, fp32_input=False, limiter=False, steps=6),
+    "cfg4_s6": dict(config=4, delta=1e-10, fp32_input=False, limiter=False, steps=6, stride=16),
 }
 
 
-def sample_indices(c, steps):
+def sample_indices(c, steps, stride=8):
     """(k, j, i) of the stored cells (docstring above).  Integer work on the config's jet geometry (R6, R7)."""
     nx, ny, nz = c["n"]
     dx, dt = c["dx"], c["dt"]
     keep = np.zeros((nz, ny, nx), bool)
-    keep[3::8, 3::8, 3::8] = True
+    keep[3::stride, 3::stride, 3::stride] = True
     for pos, d in c["jets"]:
         d = np.asarray(d, float) / np.linalg.norm(d)
         track = np.array([[np.floor((pos[a] + d[a] * s * dt + 0.5 * n * dx) / dx + 2.0 ** -20)
@@ -92,7 +92,7 @@ def run_case(name):
     U = o.get_fields(0)
     dg = o.diag()
     assert dg["has_nan"] == 0 and dg["step"] == steps
-    idx = sample_indices(c, steps)
+    idx = sample_indices(c, steps, case.get("stride", 8))
     out = os.path.join(HERE, "run_%s.npz" % name)
     np.savez(out, idx=idx, U=U[:, idx[:, 0], idx[:, 1], idx[:, 2]],
              fmax=np.abs(U).max(axis=(1, 2, 3)), fsum=U.sum(axis=(1, 2, 3), dtype=np.longdouble).astype(np.float64),
