@@ -190,7 +190,7 @@ int launch_ring_nf(hydro* h, const void* Us, int slot, int out_b, int un_b, doub
         const int nz_k = vw ? h->own_hi - h->own_lo : h->nz;              // planes the kernel sees
         RingArgs a;
         a.diag = h->diag; a.slot = slot; a.nx = h->nx; a.ny = h->ny; a.nz = nz_k; a.seg_len = h->seg_len[DIR];
-        a.eps_eff = (ORDER == 5 ? 48.0 : 144.0) * h->weno_eps; a.coef = coef; a.dt = h->dt; a.rk_a = rk_a; a.rk_b = rk_b;
+        a.eps_eff = (ORDER == 5 ? 48.0 : 144.0 / 39.0) * h->weno_eps; a.coef = coef; a.dt = h->dt; a.rk_a = rk_a; a.rk_b = rk_b;
         a.k3lam = 3.0 * h->dt / h->dx / (ORDER == 5 ? 6.0 : 12.0); a.nlim = &h->diag->nlim_total;
         a.own_lo = vw ? 0 : h->own_lo; a.own_hi = vw ? nz_k : h->own_hi;
         const int nlane = DIR == 0 ? h->ny : h->nx;

@@ -130,7 +130,7 @@ struct RingArgs {
     int nx, ny, nz;
     int seg_len;               // march cells per block (multiple of RING_CH)
     int n_long, short_nseg, short_len;   // tail-split mode (n_long >= 0), see the kernel
-    double eps_eff;            // WENO7: 144 * weno_eps (the split fluxes are carried as 2 f^+-, beta as 36 beta); WENO5: 48 * weno_eps
+    double eps_eff;            // WENO7: 144 * weno_eps / 39 (the split fluxes are carried as 2 f^+-, beta as 36 beta / 39); WENO5: 48 * weno_eps
     double coef;               // OUT_STORE / OUT_REDUCE: c = [b dt] / (2 dx);  OUT_COMBINE*: 1 / (2 dx)
     double dt, rk_a, rk_b;
     double k3lam;              // limiter: 6 dt/dx times the correction C = corr / (2 KW) (the exchange tile holds corr = KW x 2 C)
@@ -154,19 +154,26 @@ __device__ __forceinline__ int sub_off(int r, int lane) {
 
 // ------------------------------------------------------------------------------------------------ rotating window
 // Undivided differences of one split flux along the march, slot = march row mod 8:
-//   V = value, D = V - V_prev, E = sE (D - D_prev), T = E - E_prev (only the newest is kept), G = T - T_prev,
-//   S = cT T^2 + eps.  Live at any time: 4 V, 6 D, 5 E, 4 S, 3 G, 1 T (the other slots are dead registers).
-// The second differences and everything derived from them (T, G) are carried SCALED by sE = sqrt(39) (WENO7) or
-// sqrt(13) (WENO5): the smoothness indicators need 39 m^2 (13 E^2), so the scaled values enter them as plain squares --
-// one multiplication per cell instead of three per reconstruction; the linear uses of G and m fold 1/sE into FMA constants.
+//   V = value, D = V - V_prev, E = D - D_prev, T = E - E_prev, G = T - T_prev, S = cT T^2 + eps.
+// Live at any time (WENO7): 4 V, 6 D, 5 E, 4 S, 3 G, 1 T (the other slots are dead registers).
+// The kernels are issue-bound with every FP64 instruction taking two issue cycles, so the scalings are chosen
+// to leave no multiplication by a constant that an FMA coefficient can absorb:
+//   WENO7: all differences are carried UNSCALED (the push is four subtractions + S); the smoothness indicators are carried
+//          divided by 39, beta' = (lam/sqrt(39))^2 + m^2 + (39.05/39) T^2 + eps/39 -- lam is a linear form of the D's whose
+//          coefficients take the 1/sqrt(39), the m's enter as plain squares; the weights only see ratios of the betas.
+//   WENO5: the split fluxes are carried times sV = sqrt(3) (one multiplication per row), so l' = sqrt(3) l enters
+//          12 beta = 13 E^2 + 3 l^2 as a plain square; E is carried times sqrt(13) in all (one multiplication per push, factor
+//          sE = sqrt(13/3) on top of sV), the G slots hold T = E - E_prev (the candidates' differences).
 template <int ORDER> struct WinScale;
 template <> struct WinScale<7> {
     static constexpr double sE = 6.2449979983983982058, iE = 0.16012815380508713318;      // sqrt(39), 1/sqrt(39)
-    static constexpr double cT = 39.05 / 39.0;                                            // 39.05 T^2 = cT (sE T)^2
+    static constexpr double cT = 39.05 / 39.0;                                            // (39.05 T^2) / 39
+    static constexpr double sV = 1.0;
 };
 template <> struct WinScale<5> {
-    static constexpr double sE = 3.6055512754639892931, iE = 0.27735009811261456101;      // sqrt(13), 1/sqrt(13)
-    static constexpr double cT = 0.0;
+    static constexpr double sV = 1.7320508075688772935, iV = 0.57735026918962576451;      // sqrt(3), 1/sqrt(3)
+    static constexpr double sE = 2.0816659994661327353;                                   // sqrt(13/3): E carried = sqrt(13) E
+    static constexpr double iE = 0.27735009811261456101;                                  // 1/sqrt(13)
 };
 template <typename R>
 struct RotWin {
@@ -182,16 +189,20 @@ template <int r, int ORDER, typename R>
 __device__ __forceinline__ void rot_push(RotWin<R>& w, R x, R eps) {
     constexpr int p = (r + 7) & 7;
     const R dn = x - w.V[p];
-    const R en = R(WinScale<ORDER>::sE) * (dn - w.D[p]);
     if (ORDER == 7) {
+        const R en = dn - w.D[p];
         const R tn = en - w.E[p];
         w.G[r] = tn - w.T;
         w.S[r] = Real<R>::fma_(R(WinScale<7>::cT) * tn, tn, eps);
         w.T = tn;
+        w.E[r] = en;
+    } else {
+        const R en = R(WinScale<5>::sE) * (dn - w.D[p]);
+        w.G[r] = en - w.E[p];                                 // T of the WENO5 window
+        w.E[r] = en;
     }
     w.V[r] = x;
     w.D[r] = dn;
-    w.E[r] = en;
 }
 
 // reciprocal of a normal, well-scaled double: hardware seed (the upper 32 bits of the operand and of the result,
@@ -209,25 +220,26 @@ __device__ __forceinline__ float rcp_ulp(float x) {      // MUFU.RCP: 1 ulp, eno
     return r;
 }
 
-// One WENO7-JS reconstruction (r = 4) from the 1st..4th undivided differences in stencil order (D_j; E_j, G_j scaled by
-// sE = sqrt(39), see RotWin) and S_j = 39.05 T_j^2 + eps (formulas: DESIGN.md "WENO7 in difference form"):
+// One WENO7-JS reconstruction (r = 4) from the 1st..4th undivided differences in stencil order (D_j, E_j, G_j unscaled)
+// and S_j = (39.05 T_j^2 + eps) / 39 (formulas: DESIGN.md "WENO7 in difference form"):
 //   candidates   12 (q_0 - x_c) = 3 D_0 - 10 D_1 + 13 D_2,  12 (q_1-q_0) = 3 G_0,  12 (q_2-q_1) = -G_1,  12 (q_3-q_2) = G_2
-//   smoothness   36 beta_k + eps = lam_k^2 + 39 m_k^2 + S_k,
+//   smoothness   (36 beta_k + eps) / 39 = Lam_k^2 + m_k^2 + S_k,   Lam_k = lam_k / sqrt(39),
 //                lam_0 = 2 D_0 - 7 D_1 + 11 D_2, lam_1 = lam_0 + 2 G_0, lam_2 = lam_1 - G_1, lam_3 = lam_2 + 2 G_2,
 //                m_0 = 2 E_1 - E_0,  m_1 = m_2 = E_2,  m_3 = 2 E_3 - E_4
 //   weights      fp64: omega_k ~ d_k prod_{j != k} (eps + beta_j)^2,  d = (1, 12, 18, 4)/35  (common denominator;
-//                range-safe in fp64);  fp32: omega_k ~ d_k (1/(eps + beta_k))^2, one reciprocal each (R10)
-// Returns base12 = 12 (q_0 - x_c) and num12s/den = sE 12 sum_k omega_k (q_k - q_0):  W = x_c + (base12 + num12s/(sE den))/12.
+//                range-safe in fp64);  fp32: omega_k ~ d_k (1/(eps + beta_k))^2, one reciprocal each (R10);
+//                the d_k are applied as (1/4, 3, 4.5, 1): a common factor drops out of num/den
+// Returns base12 = 12 (q_0 - x_c) and num12/den = 12 sum_k omega_k (q_k - q_0):  W = x_c + (base12 + num12/den)/12.
 template <typename R>
 __device__ __forceinline__ void weno7_diff(R D0, R D1, R D2, R E0, R E1, R E2, R E3, R E4, R S0, R S1, R S2, R S3,
-                                           R G0, R G1, R G2, R& base12, R& num12s, R& den) {
+                                           R G0, R G1, R G2, R& base12, R& num12, R& den) {
     typedef Real<R> T;
     constexpr double iE = WinScale<7>::iE;
-    const R lam0 = T::fma_(R(11), D2, T::fma_(R(-7), D1, R(2) * D0));
+    const R lam0 = T::fma_(R(11 * iE), D2, T::fma_(R(-7 * iE), D1, R(2 * iE) * D0));
     const R lam1 = T::fma_(R(2 * iE), G0, lam0);
     const R lam2 = T::fma_(R(-iE), G1, lam1);
     const R lam3 = T::fma_(R(2 * iE), G2, lam2);
-    const R m0 = T::fma_(R(2), E1, -E0);                  // sE m_0, sE m_3: their squares are 39 m^2
+    const R m0 = T::fma_(R(2), E1, -E0);
     const R m3 = T::fma_(R(2), E3, -E4);
     const R b0 = T::fma_(lam0, lam0, T::fma_(m0, m0, S0));
     const R b1 = T::fma_(lam1, lam1, T::fma_(E2, E2, S1));
@@ -242,29 +254,31 @@ __device__ __forceinline__ void weno7_diff(R D0, R D1, R D2, R E0, R E1, R E2, R
         const float r0 = rcp_ulp((float)b0), r1 = rcp_ulp((float)b1), r2 = rcp_ulp((float)b2), r3 = rcp_ulp((float)b3);
         u0 = r0 * r0; u1 = r1 * r1; u2 = r2 * r2; u3 = r3 * r3;
     }
-    const R a3 = R(4) * u3;
-    const R a23 = T::fma_(R(18), u2, a3);
-    const R a123 = T::fma_(R(12), u1, a23);
-    den = u0 + a123;
-    num12s = T::fma_(a123, R(3) * G0, T::fma_(-a23, G1, a3 * G2));
-    base12 = T::fma_(R(iE), m0, lam0);                    // 3 D_0 - 10 D_1 + 13 D_2 = lam_0 + m_0 identically
+    const R a23 = T::fma_(R(4.5), u2, u3);
+    const R a123 = T::fma_(R(3), u1, a23);
+    den = T::fma_(R(0.25), u0, a123);
+    num12 = T::fma_(a123, R(3) * G0, T::fma_(-a23, G1, u3 * G2));
+    base12 = T::fma_(R(WinScale<7>::sE), lam0, m0);       // 3 D_0 - 10 D_1 + 13 D_2 = lam_0 + m_0 identically
 }
 
 // One WENO5-JS reconstruction (r = 3) from the differences of the stencil values
-// x_0..x_4 (centre x_2), D_j = x_{j+1} - x_j, E_j = D_{j+1} - D_j (carried scaled by sE = sqrt(13), see RotWin):
+// x_0..x_4 (centre x_2), D_j = x_{j+1} - x_j, E_j = D_{j+1} - D_j.  Carried (RotWin): D' = sqrt(3) D, E' = sqrt(13) E,
+// Ta = E'_1 - E'_0, Tb = E'_2 - E'_1:
 //   candidates   6 (q_0 - x_2) = 5 D_1 - 2 D_0,   6 (q_1 - q_0) = 2 (E_1 - E_0),   6 (q_2 - q_1) = -(E_2 - E_1)
-//   smoothness   12 beta_k + eps = 13 E_k^2 + 3 l_k^2 + eps,  l_0 = 3 D_1 - D_0,  l_1 = D_1 + D_2,  l_2 = 3 D_2 - D_3
-//   weights      omega_k ~ d_k / (eps + beta_k)^2,  d = (1, 6, 3)/10  (fp64: common denominator; fp32: reciprocals)
-// Returns base6 = 6 (q_0 - x_2) and num6s/den = sE 6 sum_k omega_k (q_k - q_0):  W = x_2 + (base6 + num6s/(sE den))/6.
+//   smoothness   12 beta_k + eps = E'_k^2 + l'_k^2 + eps,  l'_0 = 3 D'_1 - D'_0,  l'_1 = D'_1 + D'_2,  l'_2 = 3 D'_2 - D'_3
+//   weights      omega_k ~ d_k / (eps + beta_k)^2,  d = (1, 6, 3)/10 applied as (1/3, 2, 1)  (fp64: common denominator;
+//                fp32: reciprocals)
+// Returns base6 = 6 (q_0 - x_2) and num6s/den = sqrt(13) 6 sum_k omega_k (q_k - q_0):  W = x_2 + (base6 + num6s/(sqrt(13) den))/6.
 template <typename R>
-__device__ __forceinline__ void weno5_diff(R D0, R D1, R D2, R D3, R E0, R E1, R E2, R eps, R& base6, R& num6s, R& den) {
+__device__ __forceinline__ void weno5_diff(R D0, R D1, R D2, R D3, R E0, R E1, R E2, R Ta, R Tb, R eps, R& base6, R& num6s,
+                                           R& den) {
     typedef Real<R> T;
     const R l0 = T::fma_(R(3), D1, -D0);
     const R l1 = D1 + D2;
     const R l2 = T::fma_(R(3), D2, -D3);
-    const R b0 = T::fma_(E0, E0, T::fma_(R(3) * l0, l0, eps));
-    const R b1 = T::fma_(E1, E1, T::fma_(R(3) * l1, l1, eps));
-    const R b2 = T::fma_(E2, E2, T::fma_(R(3) * l2, l2, eps));
+    const R b0 = T::fma_(E0, E0, T::fma_(l0, l0, eps));
+    const R b1 = T::fma_(E1, E1, T::fma_(l1, l1, eps));
+    const R b2 = T::fma_(E2, E2, T::fma_(l2, l2, eps));
     R u0, u1, u2;
     if (sizeof(R) == 8) {
         const R t0 = b0 * b0, t1 = b1 * b1, t2 = b2 * b2;
@@ -273,11 +287,10 @@ __device__ __forceinline__ void weno5_diff(R D0, R D1, R D2, R D3, R E0, R E1, R
         const float r0 = rcp_ulp((float)b0), r1 = rcp_ulp((float)b1), r2 = rcp_ulp((float)b2);
         u0 = r0 * r0; u1 = r1 * r1; u2 = r2 * r2;
     }
-    const R a2 = R(3) * u2;
-    const R a12 = T::fma_(R(6), u1, a2);
-    den = u0 + a12;
-    num6s = T::fma_(a12, R(2) * (E1 - E0), -a2 * (E2 - E1));
-    base6 = T::fma_(R(5), D1, R(-2) * D0);
+    const R a12 = T::fma_(R(2), u1, u2);
+    den = T::fma_(R(1.0 / 3.0), u0, a12);
+    num6s = T::fma_(a12, R(2) * Ta, -u2 * Tb);
+    base6 = T::fma_(R(5 * WinScale<5>::iV), D1, R(-2 * WinScale<5>::iV) * D0);
 }
 
 // 2 F_hat at the interface whose newest needed cell sits in slot r of both windows (plus side lags one slot):
@@ -291,10 +304,10 @@ __device__ __forceinline__ void rot_flux_parts(const RotWin<R>& wp, const RotWin
 #define SL(k) (((r) + (k) + 16) & 7)
     R bp, np_, dp, bm, nm, dm;
     if (ORDER == 5) {
-        weno5_diff<R>(wp.D[SL(-5)], wp.D[SL(-4)], wp.D[SL(-3)], wp.D[SL(-2)], wp.E[SL(-4)], wp.E[SL(-3)], wp.E[SL(-2)], eps,
-                      bp, np_, dp);
+        weno5_diff<R>(wp.D[SL(-5)], wp.D[SL(-4)], wp.D[SL(-3)], wp.D[SL(-2)], wp.E[SL(-4)], wp.E[SL(-3)], wp.E[SL(-2)],
+                      wp.G[SL(-3)], wp.G[SL(-2)], eps, bp, np_, dp);
         weno5_diff<R>(-wm.D[SL(-1)], -wm.D[SL(-2)], -wm.D[SL(-3)], -wm.D[SL(-4)], wm.E[SL(-1)], wm.E[SL(-2)], wm.E[SL(-3)],
-                      eps, bm, nm, dm);
+                      -wm.G[SL(-1)], -wm.G[SL(-2)], eps, bm, nm, dm);
     } else {
     weno7_diff<R>(wp.D[SL(-6)], wp.D[SL(-5)], wp.D[SL(-4)],
                   wp.E[SL(-5)], wp.E[SL(-4)], wp.E[SL(-3)], wp.E[SL(-2)], wp.E[SL(-1)],
@@ -305,12 +318,13 @@ __device__ __forceinline__ void rot_flux_parts(const RotWin<R>& wp, const RotWin
                   wm.S[SL(0)], wm.S[SL(-1)], wm.S[SL(-2)], wm.S[SL(-3)],
                   wm.G[SL(0)], wm.G[SL(-1)], wm.G[SL(-2)], bm, nm, dm);
     }
-    // xs = sE (num+/den+ + num-/den-): one reciprocal for both sides in fp64
+    // xs = num+/den+ + num-/den- (WENO5: times sqrt(13)): one reciprocal for both sides in fp64
     R xs;
     if (sizeof(R) == 8) xs = (R)(fma((double)np_, (double)dm, (double)nm * (double)dp) * rcp_cubic((double)dp * (double)dm));
     else xs = (R)fmaf((float)np_, rcp_ulp((float)dp), (float)nm * rcp_ulp((float)dm));
-    corr = Real<R>::fma_(R(WinScale<ORDER>::iE), xs, bp + bm);               // KW x (high-order correction), KW = 12 or 6
-    vsum = wp.V[SL(-4)] + wm.V[SL(-3)];
+    // KW x (high-order correction), KW = 12 or 6
+    corr = ORDER == 5 ? Real<R>::fma_(R(WinScale<5>::iE), xs, bp + bm) : xs + (bp + bm);
+    vsum = wp.V[SL(-4)] + wm.V[SL(-3)];                                       // WENO5: times sV
 #undef SL
 }
 // KW x (2 F_hat) = KW vsum + corr, KW = 12 (WENO7) or 6 (WENO5): the 1/KW is folded into the divergence coefficient
@@ -318,7 +332,7 @@ template <int r, int ORDER, typename R>
 __device__ __forceinline__ R rot_flux(const RotWin<R>& wp, const RotWin<R>& wm, R eps) {
     R vsum, corr;
     rot_flux_parts<r, ORDER, R>(wp, wm, eps, vsum, corr);
-    return Real<R>::fma_(R(ORDER == 5 ? 6 : 12), vsum, corr);
+    return Real<R>::fma_(R(ORDER == 5 ? 6 * WinScale<5>::iV : 12), vsum, corr);
 }
 
 // per-thread view of one input stage: element pointers with the lane offset folded in
@@ -425,7 +439,8 @@ struct SweepCtx {
     __device__ __forceinline__ void push(const RowIn& in) {
         typedef Real<R> T;
         const R B = T::fma_(in.md, in.w, kE);
-        const R F = T::fma_(in.a, B, in.p);
+        R F = T::fma_(in.a, B, in.p);
+        if (ORDER == 5) F *= R(WinScale<5>::sV);             // alpha carries the same factor
         rot_push<r, ORDER, R>(wp, T::fma_(alpha, in.u, F), eps);
         rot_push<r, ORDER, R>(wm, T::fma_(-alpha, in.u, F), eps);
     }
@@ -617,7 +632,7 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
     cx.wp.clear();
     cx.wm.clear();
     cx.fhat_prev = R(0);
-    cx.alpha = Real<R>::from_bits(a.diag->slot[a.slot].alpha_bits[DIR]);
+    cx.alpha = Real<R>::from_bits(a.diag->slot[a.slot].alpha_bits[DIR]) * R(WinScale<ORDER>::sV);
     cx.eps = (R)a.eps_eff;
     {
         // the fluxes are carried as KW x 2 F_hat (KW = 12, 6: rot_flux); c = a.coef / KW turns their difference into the
