@@ -414,9 +414,9 @@ struct SweepCtx {
     RotWin<R> wp, wm;
     R fhat_prev;
     const R* th;                           // limiter: theta tile
-    R alpha, eps, coef, rk_a, rk_b, kE;       // coef: everything that multiplies (F_hat_prev - F_hat), see the kernel
+    R alpha, eps, coef, rk_a, rk_b;           // coef: everything that multiplies (F_hat_prev - F_hat), see the kernel
     // current chunk
-    RowPtr<DIR, R> pu, pmd, pa, pw, pp;    // own field, normal momentum, A operand, W (or zeros), P (or zeros)
+    RowPtr<DIR, R> pu, pmd, pw, pp;        // own field, normal momentum, W (energy: zeros), P (energy: M_d; else zeros)
     RowPtr<DIR, R> pus[2];                 // U_s of the output cells: rows 4..7 of the previous chunk, 0..3 of this one
     RowPtr<DIR, R> pun;                    // U^n of the output cells
     R* out;                                // this field's output sub-tile, lane offset NOT folded in
@@ -424,22 +424,21 @@ struct SweepCtx {
 
     // split fluxes of the row's cell, carried as 2 f^+- = F +- alpha U:
     //   F^d_E = M_d;  F^d_{M_j} = M_j v_d + p delta_jd;  F^d_{N_B} = N_B v_d;  v_d = M_d * W   (a-3)
-    // written branch-free as F = A * B + C with per-warp operand tiles: energy A = M_d, B = 1, C = 0;
-    // momenta / N_B: A = U_f, B = M_d W, C = p (normal component) or 0.
-    struct RowIn { R u, md, w, a, p; };
+    // written branch-free as F = U_f * (M_d * W') + C with per-warp operand tiles: momenta / N_B: W' = W, C = p (normal
+    // component) or a tile of zeros; energy: W' = zeros, C = M_d (E * 0 + M_d: four shared-memory loads per row, not five).
+    struct RowIn { R u, md, w, p; };
     template <int r>
     __device__ __forceinline__ void load(RowIn& in) const {
         in.u = pu.template at<r>();
         in.md = pmd.template at<r>();
         in.w = pw.template at<r>();
-        in.a = pa.template at<r>();
         in.p = pp.template at<r>();
     }
     template <int r>
     __device__ __forceinline__ void push(const RowIn& in) {
         typedef Real<R> T;
-        const R B = T::fma_(in.md, in.w, kE);
-        R F = T::fma_(in.a, B, in.p);
+        const R B = in.md * in.w;
+        R F = T::fma_(in.u, B, in.p);
         if (ORDER == 5) F *= R(WinScale<5>::sV);             // alpha carries the same factor
         rot_push<r, ORDER, R>(wp, T::fma_(alpha, in.u, F), eps);
         rot_push<r, ORDER, R>(wm, T::fma_(-alpha, in.u, F), eps);
@@ -644,7 +643,6 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
     cx.rk_b = (R)a.rk_b;
     cx.lane = lane;
     const bool is_energy = !BARYON && f == 0, is_normal = !BARYON && f == 1 + DIR;
-    cx.kE = is_energy ? R(1) : R(0);
 
     for (int m = 0; m < nchunks; ++m) {
         const int cm = s0 - 4 + m * RING_CH;
@@ -685,9 +683,8 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
 
         cx.pu.set(st + f * RING_SUB, lane);
         cx.pmd.set(st + (BARYON ? NF + 1 : 1 + DIR) * RING_SUB, lane);
-        cx.pa.set(is_energy ? st + (1 + DIR) * RING_SUB : st + f * RING_SUB, lane);
         cx.pw.set(is_energy ? zeros : st + NF * RING_SUB, lane);
-        cx.pp.set(is_normal ? st + (NF + 1) * RING_SUB : zeros, lane);
+        cx.pp.set(is_energy ? st + (1 + DIR) * RING_SUB : is_normal ? st + (NF + 1) * RING_SUB : zeros, lane);
         if (OUT == OUT_COMBINE1 || OUT == OUT_COMBINE) {           // the state the stage's own part is added to: U_s, or U^L
             cx.pus[0].set(LIM ? ult + ((m + 1) & 1) * NF * RING_SUB + f * RING_SUB : stp + f * RING_SUB, lane);
             cx.pus[1].set(LIM ? ult + (m & 1) * NF * RING_SUB + f * RING_SUB : st + f * RING_SUB, lane);
