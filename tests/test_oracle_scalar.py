@@ -205,6 +205,34 @@ def test_p3_weight_exponent_and_epsilon_R3(oracle):
                 assert abs(om[k] / om[0] - expect) < 1e-9 * expect, (scale, eps, k)
 
 
+def _substencil_cubic(v4):
+    """coefficients (ascending) of the cubic whose averages over the unit cells at 0, 1, 2, 3 are v4"""
+    A = np.zeros((4, 4))
+    for r in range(4):
+        for c in range(4):
+            A[r, c] = ((r + 0.5) ** (c + 1) - (r - 0.5) ** (c + 1)) / (c + 1)
+    return np.linalg.solve(A, v4)
+
+
+def test_p3_reconstructed_value_from_the_definition_R3(oracle):
+    """The VALUE the solver's reconstruction returns (oracle.weno7: the routine the interface flux calls, not the
+    diagnostic copy behind weno7_parts) is sum_k omega_k q_k with everything rebuilt here from the definition: q_k = the
+    sub-stencil cubic (given by its cell averages) at the face, beta_k = the integral definition by quadrature,
+    omega_k ~ d_k / (eps + beta_k)^2 (reading R3).  An exponent of 1 or a relative eps in the solver's routine fails this."""
+    rng = np.random.default_rng(23)
+    for scale in (1e-3, 1.0, 50.0):
+        for eps in (1e-6, 1e-2):
+            v = scale * rng.normal(size=7)
+            q = np.array([Pl.polyval(3 - k + 0.5, _substencil_cubic(v[k:k + 4])) for k in range(4)])
+            beta = np.array([_beta_from_definition(v[k:k + 4], 3 - k) for k in range(4)])
+            al = D_IDEAL / (eps + beta) ** 2
+            expect = float(al @ q / al.sum())
+            got = oracle.weno7(v, eps)
+            assert abs(got - expect) < 1e-11 * (np.max(np.abs(v)) + abs(expect)), (scale, eps, got, expect)
+            wrong = float((D_IDEAL / (eps + beta)) @ q / (D_IDEAL / (eps + beta)).sum())     # exponent 1 is distinguishable
+            assert abs(wrong - expect) > 1e-6 * np.max(np.abs(v)) or scale == 1e-3
+
+
 def _fd_derivative_error(oracle, f, dfdx, n, eps):
     """(W_{i+1/2} - W_{i-1/2})/dx vs f'(x_i) with point values f(x_i): the finite-difference use of O5-O7."""
     dx = 1.0 / n

@@ -63,6 +63,29 @@ def test_smoothness_indicators_match_integral_definition(oracle):
     assert abs(oracle.weno5(np.full(5, -1.75)) + 1.75) < 2e-15
 
 
+def test_reconstructed_value_from_the_definition(oracle):
+    """The VALUE of the solver's r = 3 reconstruction (oracle.weno5, the routine the interface flux calls; weno5_parts is a
+    diagnostic copy) is sum_k omega_k q_k rebuilt here from the definition: q_k = the sub-stencil quadratic (given by its
+    cell averages) at the face, beta_k = the integral definition, omega_k ~ d_k / (eps + beta_k)^2."""
+    rng = np.random.default_rng(29)
+    for scale in (1e-3, 1.0, 50.0):
+        for eps in (1e-6, 1e-2):
+            v = scale * rng.normal(size=5)
+            q, beta = np.zeros(3), np.zeros(3)
+            for k in range(3):
+                A = np.zeros((3, 3))
+                for r in range(3):
+                    for c in range(3):
+                        A[r, c] = ((r + 0.5) ** (c + 1) - (r - 0.5) ** (c + 1)) / (c + 1)
+                coef = np.linalg.solve(A, v[k:k + 3])
+                q[k] = Pl.polyval(2 - k + 0.5, coef)
+                beta[k] = _beta_from_definition(v[k:k + 3], 2 - k)
+            al = D5 / (eps + beta) ** 2
+            expect = float(al @ q / al.sum())
+            got = oracle.weno5(v, eps)
+            assert abs(got - expect) < 1e-11 * (np.max(np.abs(v)) + abs(expect)), (scale, eps, got, expect)
+
+
 def test_weight_limits_and_mirror(oracle):
     v = np.array([1.0, 1, 1, 5, 5])                      # step between i and i+1: sub-stencil 0 is the smooth one
     q, beta, om = oracle.weno5_parts(v)
