@@ -405,10 +405,11 @@ def main():
         from paper_1511_02137_b200 import build as B
         sha = B.source_sha()
         srows = [r for k in ("sweep_x", "sweep_y", "sweep_z") for r in rows.get(k, [])]
-        traffic = inst64 = pipe = None
+        traffic = inst64 = pipe = inst_all = None
         if srows and ncu_pass_mean(rows, "dram_read_B") is not None:
             traffic = ncu_pass_mean(rows, "dram_read_B") + ncu_pass_mean(rows, "dram_write_B")
             inst64 = ncu_pass_mean(rows, "inst_fp64")
+            inst_all = ncu_pass_mean(rows, "inst_total")
             pipe = sum(float(r["pipe_fp64_pct"]) * float(r["duration_us"]) for r in srows) / \
                 sum(float(r["duration_us"]) for r in srows) / 100.0
         avg_s = sw_ms / passes * 1e-3 if sw_n else None
@@ -429,6 +430,10 @@ def main():
                 "inst_frac": (inst64 * 64.0 / avg_s / 1e12 / peak_tf) if (inst64 and avg_s and args.precision == 64) else None,
                 "fp64_warp_inst_per_launch_ncu": inst64,
                 "fp64_pipe_busy_ncu": pipe if args.precision == 64 else None,
+                # the FP64 pipe takes a warp instruction every second issue cycle and nothing else issues in between
+                # (DESIGN.md 7): with F FP64 and O other warp-instructions a pass needs 2F + O issue cycles per scheduler,
+                # so the pipe cannot be busier than 2F / (2F + O); measured utilisation is 0.96-0.97 of this
+                "issue_ceiling_ncu": (2.0 * inst64 / (inst64 + inst_all)) if (inst64 and inst_all and args.precision == 64) else None,
                 "traffic": traffic,
                 "traffic_source": "profiles/r2_ncu_kernels.csv (ncu --set full: dram__bytes_read.sum + dram__bytes_write.sum per "
                                   "directional pass, mean over the nine passes of a step)" if srows else None,
