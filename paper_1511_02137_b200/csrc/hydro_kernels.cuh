@@ -114,10 +114,12 @@ __device__ __forceinline__ void con2prim(R E, R Mx, R My, R Mz, R e_floor, R one
         const R mx = Mx * sc, my = My * sc, mz = Mz * sc;
         M2 = mx * mx + my * my + mz * mz;
     }
+    // p = e/3 = (E^2 - M^2) / (E + s) and E + p = (2E + s)/3 (from e = s - E): ONE reciprocal serves both quotients
     const R s = T::sqrt_fast(R(4) * E * E - R(3) * M2);
-    const R e = R(3) * (E * E - M2) * T::rcp_fast(E + s);
-    p = e * R(1.0 / 3.0);
-    wt = sc * T::rcp_fast(E + p);
+    const R d1 = E + s, d2 = T::fma_(R(2), E, s);
+    const R r = T::rcp_fast(d1 * d2);
+    p = (E * E - M2) * (r * d2);
+    wt = (R(3) * sc) * (r * d1);
 }
 
 // max(|lambda_+|, |lambda_-|) of the acoustic eigenvalues along a direction with velocity component vd:
@@ -174,8 +176,13 @@ __device__ __forceinline__ void cell_speeds(R Mx, R My, R Mz, R wt, R& vx, R& vy
 }
 
 constexpr int PRIM_THREADS = 256;
+// fp64: 2 resident blocks (126 registers, no spills; 3 blocks = 80 registers spill and measure 0.146 against 0.140 ms per
+// launch at 256^3); fp32: 3 blocks.  Staging depth 2 (a third trip in flight measured the same in fp64).
+#ifndef PRIM_DEPTH
+#define PRIM_DEPTH 2
+#endif
 template <typename R>
-__global__ void __launch_bounds__(PRIM_THREADS, 3) k_prim(PrimArgs<R> a) {
+__global__ void __launch_bounds__(PRIM_THREADS, sizeof(R) == 8 ? 2 : 3) k_prim(PrimArgs<R> a) {
     R am[3] = {R(0), R(0), R(0)};
     unsigned int ncap = 0, bad = 0;
     const long long stride = (long long)gridDim.x * blockDim.x;
@@ -184,7 +191,10 @@ __global__ void __launch_bounds__(PRIM_THREADS, 3) k_prim(PrimArgs<R> a) {
     const R* __restrict__ U2 = a.U + 2 * a.Np;
     const R* __restrict__ U3 = a.U + 3 * a.Np;
     const R margin = sizeof(R) == 8 ? R(1.0 - 1e-12) : R(1.0 - 1e-5);
-    __shared__ R seed[3];
+    // one shared array: the staging slots of the main loop; before the loop its first reals hold the seeds, after it the
+    // block reduction (static shared memory is limited to 48 KB, which three trips of staging fill)
+    __shared__ __align__(16) R stg[PRIM_DEPTH][8][PRIM_THREADS];
+    R* seed = &stg[0][0][0];
     if (a.with_alpha) {
         if (threadIdx.x < 3) {
             long long cs = (long long)a.diag->slot[a.seed_slot].arg[threadIdx.x];
@@ -202,20 +212,33 @@ __global__ void __launch_bounds__(PRIM_THREADS, 3) k_prim(PrimArgs<R> a) {
     }
     R M[3] = {R(0), R(0), R(0)};
     long long arg[3] = {a.c0, a.c0, a.c0};
-    if (a.with_alpha) { M[0] = seed[0]; M[1] = seed[1]; M[2] = seed[2]; }
-    auto cell = [&](long long c, long long c0, R E, R Mx, R My, R Mz) {
-        R p, wt;
+    if (a.with_alpha) {
+        M[0] = seed[0]; M[1] = seed[1]; M[2] = seed[2];
+        __syncthreads();                                                      // before the staging loads reuse the slots
+    }
+    // 1 - v_thr^2 (shrunk a little, so that rounding can only send more cells to the full test); 2 = test every cell
+    auto om_threshold = [&]() {
+        const R cs = R(0.57735026918962576451);
+        R Mm = M[0] < M[1] ? M[0] : M[1];
+        Mm = Mm < M[2] ? Mm : M[2];
+        if (!(Mm > cs)) return R(2);
+        const R vt = (Mm - cs) / (R(1) - Mm * cs);
+        return R(1) - vt * vt * (sizeof(R) == 8 ? R(1.0 - 1e-9) : R(1.0 - 1e-4));
+    };
+    R om_thr = om_threshold();
+    auto cell = [&](long long c0, R E, R Mx, R My, R Mz, R& p, R& wt) {
         int lim;
         con2prim<R>(E, Mx, My, Mz, a.e_floor, a.one_minus_delta, p, wt, lim);
-        a.P[c] = p;
-        a.W[c] = wt;
         ncap += (c0 >= a.own_lo && c0 < a.own_hi) ? lim : 0;
-        // finite check: x - x is 0 for finite x, NaN otherwise
-        R chk = (E - E) + (Mx - Mx) + (My - My) + (Mz - Mz);
+        // finite check: 0 x is 0 for finite x, NaN otherwise
+        const R chk = Real<R>::fma_(Mz, R(0), Real<R>::fma_(My, R(0), Real<R>::fma_(Mx, R(0), E * R(0))));
         bad |= (chk == R(0)) ? 0u : 1u;
         if (!a.with_alpha) return;
         R vx, vy, vz, om, den;
         cell_speeds<R>(Mx, My, Mz, wt, vx, vy, vz, om, den);
+        // prefilter: lambda_d <= (|v| + cs) / (1 + |v| cs) in every direction (equality for v along d), so a cell with
+        // |v| <= v_thr, (v_thr + cs) / (1 + v_thr cs) = min_d M_d, cannot raise any maximum: one comparison on 1 - v^2
+        if (om >= om_thr) return;
         const R k23 = R(2.0 / 3.0), k13 = R(1.0 / 3.0);
         const R tx = Real<R>::fma_(M[0], den, -k23 * (vx < R(0) ? -vx : vx));
         const R ty = Real<R>::fma_(M[1], den, -k23 * (vy < R(0) ? -vy : vy));
@@ -236,42 +259,86 @@ __global__ void __launch_bounds__(PRIM_THREADS, 3) k_prim(PrimArgs<R> a) {
             M[0] = mx > M[0] ? mx : M[0];
             M[1] = my > M[1] ? my : M[1];
             M[2] = mz > M[2] ? mz : M[2];
+            om_thr = om_threshold();
         }
     };
     // two cells per trip, staged through thread-private shared-memory slots with cp.async, two trips deep: the loads of the
     // next trip are in flight while this trip's arithmetic runs and cost no registers (ncu of the plain loop: 40 % of the
     // issue cycles on the long scoreboard at 24 warps/SM; register double-buffering at 5 x 128 threads was slower still)
-    __shared__ R stg[2][8][PRIM_THREADS];
-    auto fetch = [&](int buf, long long cc) {
-        const long long q1 = pad_index(cc, a.nx, a.nxp), q2 = pad_index(cc + stride, a.nx, a.nxp);
-        const R* src[8] = {U0 + q1, U1 + q1, U2 + q1, U3 + q1, U0 + q2, U1 + q2, U2 + q2, U3 + q2};
+    if (a.nx == a.nxp && !(a.c0 & 1) && !(a.N & 1)) {
+        // dense rows (the usual case): the two cells of a trip are NEIGHBOURS, moved as one 2-real vector per field
+        // (16-byte cp.async / shared-memory loads / stores in fp64): half the memory instructions, 512-byte warp accesses
+        struct __align__(2 * sizeof(R)) R2 { R x, y; };
+        R2(*sv)[4][PRIM_THREADS] = reinterpret_cast<R2(*)[4][PRIM_THREADS]>(&stg[0][0][0]);
+        const long long Q = a.N >> 1;
+        auto fetchv = [&](int buf, long long q) {
+            const R* src[4] = {U0 + 2 * q, U1 + 2 * q, U2 + 2 * q, U3 + 2 * q};
 #pragma unroll
-        for (int v = 0; v < 8; ++v) {
-            const unsigned dst = (unsigned)__cvta_generic_to_shared(&stg[buf][v][threadIdx.x]);
-            if (sizeof(R) == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src[v]) : "memory");
-            else asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src[v]) : "memory");
+            for (int v = 0; v < 4; ++v) {
+                const unsigned dst = (unsigned)__cvta_generic_to_shared(&sv[buf][v][threadIdx.x]);
+                if (sizeof(R) == 8) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src[v]) : "memory");
+                else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src[v]) : "memory");
+            }
+        };
+        long long q = (a.c0 >> 1) + (long long)blockIdx.x * blockDim.x + threadIdx.x;
+        int buf = 0;
+#pragma unroll
+        for (int d = 0; d < PRIM_DEPTH - 1; ++d) {                            // PRIM_DEPTH - 1 trips in flight
+            if (q + d * stride < Q) fetchv(d, q + d * stride);
+            asm volatile("cp.async.commit_group;" ::: "memory");
         }
-    };
-    long long c = a.c0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    int buf = 0;
-    if (c + stride < a.N) fetch(0, c);
-    asm volatile("cp.async.commit_group;" ::: "memory");
-    for (; c + stride < a.N; c += 2 * stride, buf ^= 1) {
-        const long long cn = c + 2 * stride;
-        if (cn + stride < a.N) fetch(buf ^ 1, cn);
+        for (; q < Q; q += stride, buf = buf + 1 == PRIM_DEPTH ? 0 : buf + 1) {
+            const int bn = buf == 0 ? PRIM_DEPTH - 1 : buf - 1;               // the slot the previous trip has just freed
+            if (q + (PRIM_DEPTH - 1) * stride < Q) fetchv(bn, q + (PRIM_DEPTH - 1) * stride);
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            asm volatile("cp.async.wait_group %0;" ::"n"(PRIM_DEPTH - 1) : "memory");   // this trip's four vectors have landed
+            const R2 E = sv[buf][0][threadIdx.x], Mx = sv[buf][1][threadIdx.x], My = sv[buf][2][threadIdx.x],
+                     Mz = sv[buf][3][threadIdx.x];
+            R2 p, w;
+            cell(2 * q, E.x, Mx.x, My.x, Mz.x, p.x, w.x);
+            cell(2 * q + 1, E.y, Mx.y, My.y, Mz.y, p.y, w.y);
+            *reinterpret_cast<R2*>(a.P + 2 * q) = p;
+            *reinterpret_cast<R2*>(a.W + 2 * q) = w;
+        }
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+    } else {
+        auto fetch = [&](int buf, long long cc) {
+            const long long q1 = pad_index(cc, a.nx, a.nxp), q2 = pad_index(cc + stride, a.nx, a.nxp);
+            const R* src[8] = {U0 + q1, U1 + q1, U2 + q1, U3 + q1, U0 + q2, U1 + q2, U2 + q2, U3 + q2};
+#pragma unroll
+            for (int v = 0; v < 8; ++v) {
+                const unsigned dst = (unsigned)__cvta_generic_to_shared(&stg[buf][v][threadIdx.x]);
+                if (sizeof(R) == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src[v]) : "memory");
+                else asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src[v]) : "memory");
+            }
+        };
+        long long c = a.c0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;
+        int buf = 0;
+        if (c + stride < a.N) fetch(0, c);
         asm volatile("cp.async.commit_group;" ::: "memory");
-        asm volatile("cp.async.wait_group 1;" ::: "memory");                  // this trip's eight values have landed
-        const R E = stg[buf][0][threadIdx.x], Mx = stg[buf][1][threadIdx.x], My = stg[buf][2][threadIdx.x],
-                Mz = stg[buf][3][threadIdx.x];
-        const R E2 = stg[buf][4][threadIdx.x], Mx2 = stg[buf][5][threadIdx.x], My2 = stg[buf][6][threadIdx.x],
-                Mz2 = stg[buf][7][threadIdx.x];
-        cell(pad_index(c, a.nx, a.nxp), c, E, Mx, My, Mz);
-        cell(pad_index(c + stride, a.nx, a.nxp), c + stride, E2, Mx2, My2, Mz2);
-    }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
-    if (c < a.N) {
-        const long long p1 = pad_index(c, a.nx, a.nxp);
-        cell(p1, c, U0[p1], U1[p1], U2[p1], U3[p1]);
+        for (; c + stride < a.N; c += 2 * stride, buf ^= 1) {
+            const long long cn = c + 2 * stride;
+            if (cn + stride < a.N) fetch(buf ^ 1, cn);
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            asm volatile("cp.async.wait_group 1;" ::: "memory");              // this trip's eight values have landed
+            const R E = stg[buf][0][threadIdx.x], Mx = stg[buf][1][threadIdx.x], My = stg[buf][2][threadIdx.x],
+                    Mz = stg[buf][3][threadIdx.x];
+            const R E2 = stg[buf][4][threadIdx.x], Mx2 = stg[buf][5][threadIdx.x], My2 = stg[buf][6][threadIdx.x],
+                    Mz2 = stg[buf][7][threadIdx.x];
+            const long long p1 = pad_index(c, a.nx, a.nxp), p2 = pad_index(c + stride, a.nx, a.nxp);
+            R p, w;
+            cell(c, E, Mx, My, Mz, p, w);
+            a.P[p1] = p; a.W[p1] = w;
+            cell(c + stride, E2, Mx2, My2, Mz2, p, w);
+            a.P[p2] = p; a.W[p2] = w;
+        }
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        if (c < a.N) {
+            const long long p1 = pad_index(c, a.nx, a.nxp);
+            R p, w;
+            cell(c, U0[p1], U1[p1], U2[p1], U3[p1], p, w);
+            a.P[p1] = p; a.W[p1] = w;
+        }
     }
     // warp reduction by shuffles, then one atomic per block on the bit pattern (non-negative reals order like
     // unsigned integers; the max is exact, hence order independent)
@@ -289,7 +356,8 @@ __global__ void __launch_bounds__(PRIM_THREADS, 3) k_prim(PrimArgs<R> a) {
         ncap += __shfl_xor_sync(0xffffffffu, ncap, off);
         bad |= __shfl_xor_sync(0xffffffffu, bad, off);
     }
-    __shared__ unsigned long long sm[8][8];
+    __syncthreads();                                                          // every thread is done with its staging slots
+    unsigned long long(*sm)[8] = reinterpret_cast<unsigned long long(*)[8]>(&stg[0][0][0]);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (lane == 0) {
         sm[warp][0] = ab[0]; sm[warp][1] = ab[1]; sm[warp][2] = ab[2]; sm[warp][3] = ncap; sm[warp][4] = bad;
@@ -374,8 +442,13 @@ __device__ __forceinline__ R low_term(const LowCell<R, NF>& x, int d, int q, R s
     return F - s_alpha * x.u[q];
 }
 
+// 4 resident blocks (64 registers, no spills): 0.336 -> 0.305 ms at 256^3; 3 blocks (80 registers) and a second plane of
+// prefetch (plane k + 2 in flight for a whole trip) both measured slower -- the kernel waits on L1/L2, not on DRAM latency
+#ifndef LOWUP_BLOCKS
+#define LOWUP_BLOCKS 4
+#endif
 template <typename R, int NF>
-__global__ void __launch_bounds__(256) k_lowup(LowArgs<R> a, int seg_len) {
+__global__ void __launch_bounds__(256, LOWUP_BLOCKS) k_lowup(LowArgs<R> a, int seg_len) {
     typedef Real<R> T;
     R alpha[3];
 #pragma unroll

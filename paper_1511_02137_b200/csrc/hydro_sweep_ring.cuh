@@ -355,18 +355,20 @@ struct RowPtr {
 };
 
 // ------------------------------------------------------------------------------------------------ limiter (R16, f-1)
-// theta of one cell for the face state W1 = W0 + sgn * a (W0 = U^L of the cell, a = 6 dt/dx C of the face):
-// 1 if g(W1) >= delta, else (g(W0) - delta) / (g(W0) - g(W1)), g = E - |M|, delta = min(1e-8 E0, g(W0)).
-// The common case is decided on squares (no square root).
+// theta of one cell for the face state W1 = W0 + ks * c (W0 = U^L of the cell, c = the face's correction in the exchange
+// tile, ks = +-6 dt/dx / (2 KW)): 1 if g(W1) >= delta, else (g(W0) - delta) / (g(W0) - g(W1)), g = E - |M|,
+// delta = min(1e-8 E0, g(W0)).  Common case, decided on squares without looking at g(W0): delta <= 1e-8 E0, so
+// g(W1) >= 1e-8 E0 already gives theta = 1.
 template <typename R>
-__device__ __forceinline__ R theta_cell(const R W0[4], const R a[4], R sgn) {
-    const R E0 = W0[0], M02 = W0[1] * W0[1] + W0[2] * W0[2] + W0[3] * W0[3];
+__device__ __forceinline__ R theta_cell(const R W0[4], const R c[4], R ks) {
+    const R E0 = W0[0];
     const R d8 = R(1e-8) * E0;
-    const R W1[4] = {Real<R>::fma_(sgn, a[0], W0[0]), Real<R>::fma_(sgn, a[1], W0[1]), Real<R>::fma_(sgn, a[2], W0[2]),
-                     Real<R>::fma_(sgn, a[3], W0[3])};
+    const R W1[4] = {Real<R>::fma_(ks, c[0], W0[0]), Real<R>::fma_(ks, c[1], W0[1]), Real<R>::fma_(ks, c[2], W0[2]),
+                     Real<R>::fma_(ks, c[3], W0[3])};
     const R M12 = W1[1] * W1[1] + W1[2] * W1[2] + W1[3] * W1[3];
-    const R t0 = E0 - d8, t1 = W1[0] - d8;
-    if (t0 >= R(0) && t0 * t0 >= M02 && t1 >= R(0) && t1 * t1 >= M12) return R(1);
+    const R t1 = W1[0] - d8;
+    if (t1 >= R(0) && t1 * t1 >= M12) return R(1);
+    const R M02 = W0[1] * W0[1] + W0[2] * W0[2] + W0[3] * W0[3];
     const R g0 = E0 - Real<R>::sqrt_(M02), g1 = W1[0] - Real<R>::sqrt_(M12);
     const R delta = d8 < g0 ? d8 : g0;
     if (g1 >= delta) return R(1);
@@ -386,7 +388,7 @@ __device__ __noinline__ int theta_row(int r, const R* st, const R* stp, const R*
     const int o = sub_off<DIR, R>(r, lane);
     R a[4];
 #pragma unroll
-    for (int q = 0; q < 4; ++q) a[q] = k3lam * xc_all[q * RING_SUB + o];
+    for (int q = 0; q < 4; ++q) a[q] = xc_all[q * RING_SUB + o];
     const int i = cm + r - 4;
     R theta = R(1);
     if (i >= 0 && i <= nd - 1) {
@@ -394,7 +396,7 @@ __device__ __noinline__ int theta_row(int r, const R* st, const R* stp, const R*
         const R* s = r < 4 ? stp : st;
         const int ol = sub_off<DIR, R>(rl, lane);
         const R W0[4] = {s[ol], s[RING_SUB + ol], s[2 * RING_SUB + ol], s[3 * RING_SUB + ol]};
-        const R t = theta_cell<R>(W0, a, R(-1));
+        const R t = theta_cell<R>(W0, a, -k3lam);
         theta = t < theta ? t : theta;
     }
     if (i + 1 >= 0 && i + 1 <= nd - 1) {
@@ -402,7 +404,7 @@ __device__ __noinline__ int theta_row(int r, const R* st, const R* stp, const R*
         const R* s = r < 3 ? stp : st;
         const int orr = sub_off<DIR, R>(rr, lane);
         const R W0[4] = {s[orr], s[RING_SUB + orr], s[2 * RING_SUB + orr], s[3 * RING_SUB + orr]};
-        const R t = theta_cell<R>(W0, a, R(1));
+        const R t = theta_cell<R>(W0, a, k3lam);
         theta = t < theta ? t : theta;
     }
     th[o] = theta;
