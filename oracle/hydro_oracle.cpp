@@ -283,7 +283,7 @@ struct Oracle {
     long long ncap;
     int has_nan;
     double deposited[4];
-    double last_q[3][16];           // q per stage for up to 16 jets (for the P5 pin)
+    double last_q[3][64];           // q per stage for up to 64 jets (the P5 pin and the deposited totals; eq. (2) sums over all jets)
     size_t N() const { return (size_t)nx * ny * nz; }
     size_t idx(int i, int j, int k) const { return ((size_t)k * ny + j) * nx + i; }
 };
@@ -525,7 +525,7 @@ void eval_rhs(Oracle& o, const std::vector<double>& U, double stage_c, std::vect
                 }
             }
         }
-        if (J < 16 && stage_no >= 0) o.last_q[stage_no][J] = q;
+        if (J < 64 && stage_no >= 0) o.last_q[stage_no][J] = q;
     }
 }
 
@@ -540,7 +540,7 @@ void rk3_step(Oracle& o) {
     eval_rhs(o, o.U2, 0.5, o.L, 2, true);
     for (size_t n = 0; n < T; ++n) o.U[n] = (1.0 / 3.0) * o.U[n] + (2.0 / 3.0) * (o.U2[n] + dt * o.L[n]);
     const double w[3] = {1.0 / 6.0, 1.0 / 6.0, 2.0 / 3.0};   // effective weights (R5)
-    for (size_t J = 0; J < o.jets.size() && J < 16; ++J)
+    for (size_t J = 0; J < o.jets.size() && J < 64; ++J)
         for (int s = 0; s < 3; ++s) {
             double a = dt * w[s] * o.last_q[s][J];
             o.deposited[0] += a;
@@ -647,7 +647,7 @@ void oracle_eval_rhs(void* h, double stage_c, double* out) {
 // the three stage values q^s of every jet during the LAST step (P5 pin): out[3*njets], s-major
 void oracle_last_stage_q(void* h, double* out) {
     Oracle* o = (Oracle*)h;
-    size_t nj = std::min<size_t>(o->jets.size(), 16);
+    size_t nj = std::min<size_t>(o->jets.size(), 64);
     for (int s = 0; s < 3; ++s) for (size_t J = 0; J < nj; ++J) out[s * nj + J] = o->last_q[s][J];
 }
 

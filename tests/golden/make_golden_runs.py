@@ -15,6 +15,8 @@ Cases (name: config, steps, oracle options):
     cfg3_fp32     config 3 with the fp32 variant's reading R10: initial state rounded to fp32, delta = 1e-5
     cfg3_lim      config 3 with the positivity-preserving flux limiter (reading R16)
     cfg3_w5       config 3 with the WENO5 variant, 120 steps
+    cfg2_s500     config 2 run ten times its length (500 steps, t = 10 fm/c): the jet crosses the whole grid and LEAVES it through
+                  the +x face at step ~470 (a jet outside deposits nothing, R7), the flow reaches the outflow boundaries
     cfg4_s6       BASELINE config 4 at FULL SIZE (512^3, nf = 5, two jets), the first 6 of its 200 steps (the whole run is
                   ~4 h of oracle time; 6 steps are ~10 min and ~40 GB) -- the one oracle comparison at the size where the
                   nf = 5 kernels run several waves with tail splitting
@@ -47,6 +49,7 @@ CASES = {
     "cfg3_fp32": dict(config=3, delta=1e-5, fp32_input=True, limiter=False),
     "cfg3_lim": dict(config=3, delta=1e-10, fp32_input=False, limiter=True),
     "cfg3_w5": dict(config=3, delta=1e-10, fp32_input=False, limiter=False, weno_order=5),
+    "cfg2_s500": dict(config=2, delta=1e-10, fp32_input=False, limiter=False, steps=500),
     "cfg4_s6": dict(config=4, delta=1e-10, fp32_input=False, limiter=False, steps=6, stride=16),
 }
 

@@ -138,6 +138,36 @@ def test_jet_cell_and_source_bitwise_location(H, oracle):
             x.close()
 
 
+def test_maximum_number_of_jets(H, oracle):
+    """Eq. (2) sums over jets: a full jet table (64, the handle's maximum), seeded positions and directions,
+    several jets starting next to a face and leaving the grid during the run (a jet outside deposits nothing, R7), compared
+    with the oracle after 8 steps; the 65th jet is refused with HYDRO_ESTATE and leaves the table unchanged."""
+    c = S.scaled_config(0, (32, 24, 20))
+    rng = np.random.default_rng(64)
+    half = 0.5 * np.array(c["n"]) * c["dx"]
+    jets = []
+    for j in range(64):
+        pos = rng.uniform(-0.9, 0.9, size=3) * half
+        d = rng.normal(size=3)
+        if j % 8 == 0:                                   # next to the +x face, heading out: gone after a few steps
+            pos[0] = half[0] - 0.05
+            d = np.array([1.0, 0.1 * d[1], 0.1 * d[2]])
+        jets.append((tuple(pos), tuple(d)))
+    c["jets"] = jets
+    _, U0, g, o = make_pair(H, oracle, c)
+    with pytest.raises(H.HydroError) as ei:
+        g.add_jet((0.0, 0.0, 0.0), (1.0, 0.0, 0.0))
+    assert ei.value.code == H.ESTATE
+    g.step(8)
+    o.step(8)
+    errs = r13(g.get_fields(), o.get_fields())
+    assert max(errs) < 1e-9, errs
+    dg, do = compare_diag(g, o, 8)
+    assert dg["deposited"][0] > 0
+    g.close()
+    o.close()
+
+
 # ------------------------------------------------------------------------------------------------ whole path
 def test_config0_full_run(H, oracle):
     c, U0, g, o = make_pair(H, oracle, 0)
