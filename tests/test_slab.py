@@ -155,6 +155,39 @@ def test_slabs_match_the_single_handle_run_bitwise(H, case):
         sl.close()
 
 
+@pytest.mark.gpu
+def test_slab_run_of_config2_matches_the_oracle_sample(H):
+    """The decomposed path against the ORACLE directly (not only against the one-handle run): BASELINE config 2 (128^3, jet)
+    for its full 50 steps as 4 z-slabs in the overlapped schedule, compared with the stored final state of the oracle run
+    (tests/golden/run_cfg2.npz, written by make_golden_runs.py from oracle/ only) at 1e-9 (north_star)."""
+    import torch
+    gold = np.load(os.path.join(ROOT, "tests", "golden", "run_cfg2.npz"))
+    c = S.CONFIGS[2]
+    steps, world = int(gold["steps"]), 4
+    assert steps == c["steps"]
+    U0 = S.make_state(2)
+    st = torch.cuda.Stream()
+    slabs = [SL.Slab(H, c["n"], c["dx"], c["dt"], r, world, stream=st) for r in range(world)]
+    for sl in slabs:
+        sl.set_state(U0)
+        for pos, d in c["jets"]:
+            sl.g.add_jet(pos, d, S.KAPPA_RAD, S.KAPPA_COLL, S.CR_OVER_CF)
+    SL.run_local(slabs, steps)
+    U = np.concatenate([sl.owned() for sl in slabs], axis=1)
+    idx = gold["idx"]
+    errs = np.max(np.abs(U[:, idx[:, 0], idx[:, 1], idx[:, 2]] - gold["U"]), axis=1) / gold["fmax"]
+    assert np.all(errs < 1e-9), errs
+    fsum = U.sum(axis=(1, 2, 3), dtype=np.longdouble).astype(np.float64)
+    assert np.all(np.abs(fsum - gold["fsum"]) <= 1e-11 * gold["fabs"])
+    ds = [sl.g.diag() for sl in slabs]
+    assert abs(sum(d["ncap"] for d in ds) - int(gold["ncap"])) <= max(2, 0.02 * int(gold["ncap"]))
+    assert np.max(np.abs(np.max([d["alpha"] for d in ds], axis=0) - gold["alpha"])) < 1e-12
+    dep = sum(d["deposited"] for d in ds)
+    assert np.max(np.abs(dep - gold["deposited"])) <= 1e-10 * gold["deposited"][0]
+    for sl in slabs:
+        sl.close()
+
+
 def _rank_main(rank, world, port, case, q):
     """One process = one rank with its own CUDA context and Slab handle on the ONE GPU; torch.distributed over gloo."""
     sys.path.insert(0, ROOT)
