@@ -168,6 +168,26 @@ def test_maximum_number_of_jets(H, oracle):
     o.close()
 
 
+def test_jet_added_in_the_middle_of_a_run(H, oracle):
+    """The path length of eq. (3) counts from the step a jet was added (R8: l = t - t_added): a second jet added after
+    two steps (the captured step graph is rebuilt for the new jet table), three more steps, compared with the oracle."""
+    c = S.scaled_config(0, (32, 24, 20))
+    _, U0, g, o = make_pair(H, oracle, c)
+    g.step(2)
+    o.step(2)
+    for x in (g, o):
+        x.add_jet((0.4, -0.3, 0.2), (-0.6, 0.7, 0.1), 3.0, 1.5, 9.0 / 4.0)
+    g.step(3)
+    o.step(3)
+    errs = r13(g.get_fields(), o.get_fields())
+    assert max(errs) < 1e-9, errs
+    compare_diag(g, o, 5)
+    qg, qo = g.last_stage_q(), o.last_stage_q()
+    assert qg.shape == qo.shape == (3, 2) and np.max(np.abs(qg - qo)) < 1e-11 * np.max(qo)
+    g.close()
+    o.close()
+
+
 # ------------------------------------------------------------------------------------------------ whole path
 def test_config0_full_run(H, oracle):
     c, U0, g, o = make_pair(H, oracle, 0)
