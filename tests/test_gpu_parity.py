@@ -721,6 +721,32 @@ def test_checkpoint_resume_is_bitwise(H):
     g.close(), r.close()
 
 
+def test_non_finite_state_is_flagged(H, oracle):
+    """has_nan: a NaN or an infinity in any conserved field of any cell is flagged by k_prim (0 * x summed over the fields),
+    like the oracle does; ragged and dense grids (the scalar and the vector path of k_prim), both precisions."""
+    for n in ((6, 5, 4), (7, 5, 3), (32, 8, 8)):
+        c = S.scaled_config(0, n)
+        U0 = S.make_state(c, noise=False)
+        for prec in (64, 32):
+            for f, cell, bad in ((None, None, None), (0, (0, 0, 0), np.nan), (1, (n[2] - 1, n[1] - 1, n[0] - 1), np.inf),
+                                 (2, (1, 2, 3), -np.inf), (3, (2, 0, 1), np.nan)):
+                U = U0.copy()
+                if f is not None:
+                    U[(f,) + cell] = bad
+                g = H.Hydro(*n, c["dx"], c["dt"], precision=prec)
+                g.set_state(U.astype(np.float64 if prec == 64 else np.float32))
+                g.step(1)                                    # the flag is committed with the stages of a step
+                flag = g.diag()["has_nan"]
+                g.close()
+                if prec == 64:
+                    o = oracle.Oracle(*n, c["dx"], c["dt"])
+                    o.set_state(U)
+                    o.eval_rhs(0.0)
+                    assert o.diag()["has_nan"] == (0 if f is None else 1)
+                    o.close()
+                assert flag == (0 if f is None else 1), (n, prec, f, cell, bad)
+
+
 def test_error_paths(H):
     g = H.Hydro(8, 8, 8, 0.1, 0.02)
     with pytest.raises(H.HydroError):

@@ -229,3 +229,23 @@ def test_p8_rk3_source_stage_times_and_quadrature(oracle):
     gained = (o.get_fields(0)[0].sum(dtype=np.longdouble) - U0[0].sum(dtype=np.longdouble)) * dx ** 3
     assert abs(float(gained) / s - (B * t + 0.5 * A * t * t)) < 1e-5 * B * t
     o.close()
+
+
+def test_non_finite_state_is_flagged_per_field_and_cell(oracle):
+    """Diagnostics: a NaN or an infinity in any conserved field of any cell raises has_nan; a finite state does not."""
+    n = (6, 5, 4)
+    c = S.scaled_config(0, n)
+    U0 = S.make_state(c, noise=False)
+    o = oracle.Oracle(*n, c["dx"], c["dt"])
+    o.set_state(U0)
+    o.eval_rhs(0.0)
+    assert o.diag()["has_nan"] == 0
+    o.close()
+    for f, cell, bad in ((0, (0, 0, 0), np.nan), (1, (3, 4, 5), np.inf), (2, (1, 2, 3), -np.inf), (3, (2, 0, 1), np.nan)):
+        U = U0.copy()
+        U[(f,) + cell] = bad
+        o = oracle.Oracle(*n, c["dx"], c["dt"])
+        o.set_state(U)
+        o.eval_rhs(0.0)
+        assert o.diag()["has_nan"] == 1, (f, cell, bad)
+        o.close()
