@@ -291,6 +291,8 @@ class Hydro:
         return out
 
     def diag(self):
+        """hydro_get_diag.  ncap, has_nan and deposited are committed by the stages of step() (and of the stage_* calls);
+        eval_rhs() refreshes alpha only."""
         alpha = (C.c_double * 3)()
         dep = (C.c_double * 4)()
         cfl, ncap, nan, step = C.c_double(), C.c_longlong(), C.c_int(), C.c_longlong()
