@@ -126,7 +126,10 @@ def test_jet_cell_and_source_bitwise_location(H, oracle):
     """The deposit cell is integer work: the set of cells touched by the source must be identical."""
     c = S.scaled_config(0, (24, 20, 16))
     c["jets"] = [((0.0, 0.0, 0.0), (1.0, 0.0, 0.0)), ((0.0, 0.0, 0.0), (-1.0, 0.0, 0.0)),
-                 ((-0.35, 0.25, 0.05), (0.3, -0.4, 0.2)), ((9.0, 0.0, 0.0), (1.0, 0.0, 0.0))]
+                 ((-0.35, 0.25, 0.05), (0.3, -0.4, 0.2)), ((9.0, 0.0, 0.0), (1.0, 0.0, 0.0)),
+                 # 0.8 and 1.2 x 2^-20 cells below a face: the upper / the lower cell (size of the R7 bias), at rest along x
+                 ((0.3 - 0.8 * 2.0 ** -20 * 0.1, -0.45, 0.33), (0.0, 1e-9, 1.0)),
+                 ((0.3 - 1.2 * 2.0 ** -20 * 0.1, 0.45, -0.33), (0.0, 1e-9, -1.0))]
     for stage_c in (0.0, 0.5, 1.0):
         _, U0, g, o = make_pair(H, oracle, c)
         _, _, g0, o0 = make_pair(H, oracle, c, jets=False)

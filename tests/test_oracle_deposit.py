@@ -139,6 +139,18 @@ def test_jet_moves_along_its_direction_at_c_and_leaves_the_grid(oracle):
                 assert np.max(np.abs(com - pos)) < 0.02 * dx + 2e-3, (stage_c, com, pos)
         seen.add(cell)
     assert len(seen) == 5                                     # five different cells along the track
+    # a jet sitting in the FIRST cell of an axis (index 0) deposits like any other
+    for axis in range(3):
+        pos = np.array([0.03, -0.02, 0.01])
+        pos[axis] = -0.5 * n[axis] * dx + 0.4 * dx
+        o = oracle.Oracle(*n, dx, dt)
+        o.set_state(U0)
+        L0 = o.eval_rhs(0.0)
+        o.add_jet(tuple(pos), (0.0, 0.0, 1.0) if axis != 2 else (1.0, 0.0, 0.0))
+        dL = o.eval_rhs(0.0) - L0
+        o.close()
+        nz = np.argwhere(dL[0] != 0)
+        assert len(nz) == 1 and tuple(nz[0][::-1]) == _r7_cell(pos, n, dx) and nz[0][::-1][axis] == 0
     # outside: nothing is deposited, q = 0, the deposited totals do not move
     o = oracle.Oracle(*n, dx, dt)
     o.set_state(U0)

@@ -5,6 +5,7 @@ built on and the properties it must deliver, not the oracle's own formulas:
   * with the limiter the state stays admissible (g = E - |M| > 0) where the unlimited scheme does not;
   * smooth data: theta = 1 everywhere, i.e. the scheme is unchanged; conservation and symmetry are untouched."""
 import numpy as np
+import pytest
 
 from paper_1511_02137_b200 import synthetic as S
 
@@ -144,7 +145,8 @@ def _weno7_from_definition(v, eps):
     return float(a @ q / a.sum())
 
 
-def test_r16_constants_on_a_linear_admissibility_function(oracle):
+@pytest.mark.parametrize("seed,span,vlo,small", [(3, 0.5, 0.6, False), (4, 1.0, 0.3, True)])
+def test_r16_constants_on_a_linear_admissibility_function(oracle, seed, span, vlo, small):
     """Reading R16 states: the limited Euler update is the average of the six states
     W_f = U^L_i -+ 6 (dt/dx) theta_f C_f, and theta_f is the largest value for which g(W_f) >= delta_i =
     min(1e-8 E^L_i, g(U^L_i)) in both cells of the face, as far as the concavity of g = E - |M| can tell.  In 1-D with
@@ -154,12 +156,13 @@ def test_r16_constants_on_a_linear_admissibility_function(oracle):
     of the reconstruction.  On the remaining limited faces (M_x changes sign: g is only concave) the oracle's theta must
     be admissible and not larger than the supremum.  The oracle's face fluxes are recovered from its L by summing the
     divergence from the left boundary, where a uniform pad makes the flux known.  A different face multiplier
-    (6 -> 12) or a different delta (1e-8 -> 1e-4) moves theta on the linear faces and fails this test."""
+    (6 -> 12) or a different delta (1e-8 -> 1e-4) moves theta on the linear faces and fails this test.  The second, rougher
+    parameter set reaches theta < 0.25 on linear faces (a theta clipped or floored there would go unnoticed otherwise)."""
     nx, pad, dx, dt, eps = 72, 6, 0.1, 0.02, 1e-6
     lam = dt / dx
-    rng = np.random.default_rng(3)
-    e = 10.0 ** rng.uniform(-0.5, 0.5, nx)
-    v = rng.uniform(0.6, 0.985, nx)
+    rng = np.random.default_rng(seed)
+    e = 10.0 ** rng.uniform(-span, span, nx)
+    v = rng.uniform(vlo, 0.985, nx)
     e[:pad], v[:pad] = e[pad], v[pad]                     # uniform pad: the flux through the left boundary is F(U_0)
     gam2 = 1.0 / (1.0 - v * v)
     E = (4.0 / 3.0) * e * gam2 - e / 3.0                  # eq. (1), p = e/3
@@ -198,6 +201,7 @@ def test_r16_constants_on_a_linear_admissibility_function(oracle):
             linear[f] = all(UL[1, c] > 0 and UL[1, c] + sgn * 6.0 * lam * C[1, f] > 0 for c, sgn in cells(f))
     lim = theta < 1.0
     assert np.sum(lim & linear & (theta > 0.05) & (theta < 0.95)) >= 4      # the case must exercise the exact regime
+    assert not small or np.sum(lim & linear & (theta > 0.02) & (theta < 0.25)) >= 1
     o = oracle.Oracle(nx, 1, 1, dx, dt)
     U4 = np.zeros((4, 1, 1, nx))
     U4[0, 0, 0], U4[1, 0, 0] = E, M
@@ -224,3 +228,34 @@ def test_r16_constants_on_a_linear_admissibility_function(oracle):
         else:
             assert -1e-9 <= th_o <= theta[f] + 1e-8 and admissible(f, max(th_o, 0.0), slack=1e-9), (f, th_o, theta[f])
     o.close()
+
+
+def test_limiter_is_mirror_symmetric_on_rough_data_up_to_the_boundary_cells(oracle):
+    """x -> -x (reverse the line, flip the sign of M_x) must mirror the limited RHS, boundary cells included: ghost cells
+    impose no admissibility condition, the first and the last interior cell do (P6 with the limiter active everywhere)."""
+    nx, dx, dt = 40, 0.1, 0.02
+    nlim = 0
+    for seed in range(8):
+        rng = np.random.default_rng(100 + seed)
+        e = 10.0 ** rng.uniform(-1.0, 1.0, nx)
+        v = rng.uniform(-0.98, 0.98, nx)
+        gam2 = 1.0 / (1.0 - v * v)
+        U = np.zeros((4, 1, 1, nx))
+        U[0, 0, 0] = (4.0 / 3.0) * e * gam2 - e / 3.0
+        U[1, 0, 0] = (4.0 / 3.0) * e * gam2 * v
+        Um = U[..., ::-1].copy()
+        Um[1] = -Um[1]
+        out = []
+        for W in (U, Um):
+            o = oracle.Oracle(nx, 1, 1, dx, dt)
+            o.set_state(W)
+            o.set_limiter(True)
+            out.append((o.eval_rhs(0.0), o.limited_faces()))
+            o.close()
+        (L, n1), (Lm, n2) = out
+        assert n1 == n2
+        nlim += n1
+        scale = np.max(np.abs(L), axis=(1, 2, 3))
+        assert np.max(np.abs(Lm[0] - L[0][..., ::-1])) < 1e-11 * scale[0]
+        assert np.max(np.abs(Lm[1] + L[1][..., ::-1])) < 1e-11 * scale[1]
+    assert nlim > 40

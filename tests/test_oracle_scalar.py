@@ -331,6 +331,11 @@ def test_r7_jet_cell_index(oracle):
     assert oracle.jet_axis_index(0.05, n, dx) == 16
     assert oracle.jet_axis_index(-0.05, n, dx) == 15
     assert oracle.jet_axis_index(1.61, n, dx) == -1 and oracle.jet_axis_index(-1.61, n, dx) == -1
+    # the size of the bias: a position 0.8 x 2^-20 cells below a face counts as the upper cell, 1.2 x 2^-20 cells below
+    # it as the lower one (rounding of (x - x_min)/dx is ~1e-15 cells, far below 0.2 x 2^-20)
+    for face, i in ((-0.3, 13), (0.7, 23), (0.0, 16)):
+        assert oracle.jet_axis_index(face - 0.8 * 2.0 ** -20 * dx, n, dx) == i
+        assert oracle.jet_axis_index(face - 1.2 * 2.0 ** -20 * dx, n, dx) == i - 1
     # every stage position of the BASELINE jets is at least 0.05 cells away from a rounding-sensitive tie
     for x0, nn in [(-1.0, 32), (-3.0, 128), (-5.0, 256)]:
         for step in range(0, 60):
