@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhydro.so")
 SOURCES = [os.path.join(CSRC, "hydro.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "hydro_kernels.cuh"), os.path.join(CSRC, "hydro_sweep_ring.cuh"),
+DEPS = SOURCES + [os.path.join(CSRC, "hydro_kernels.cuh"), os.path.join(CSRC, "hydro_sweep_ring.cuh"), os.path.join(CSRC, "hydro_lowup.cuh"),
                   os.path.join(os.path.dirname(HERE), "include", "hydro.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--fmad=true",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v", "-lcudart"]

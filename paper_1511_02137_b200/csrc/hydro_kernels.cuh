@@ -417,19 +417,10 @@ struct LowArgs {
     R lam;                       // dt / dx
 };
 
-// Launch: block (32, 8) = a tile of 32 x 8 columns, grid (ceil(nx/32), ceil(ny/8), z segments); every thread marches its
-// column along z keeping the cell below / at / above in registers (the z neighbours cost no loads); the four in-plane
-// neighbours are L1 hits (they are the plane the block's own threads loaded one trip earlier).
+// one cell's inputs of the first-order update (the kernel is k_lowup_tma, hydro_lowup.cuh)
 template <typename R, int NF>
 struct LowCell { R u[NF], w, p; };
 
-template <typename R, int NF>
-__device__ __forceinline__ void low_load(const LowArgs<R>& a, long long c, LowCell<R, NF>& x) {
-#pragma unroll
-    for (int q = 0; q < NF; ++q) x.u[q] = a.U[q * a.Np + c];
-    x.w = a.W[c];
-    x.p = a.P[c];
-}
 // (F^d_q - s alpha U_q) of a cell, s = +1 (upper neighbour) or -1 (lower neighbour)
 template <typename R, int NF>
 __device__ __forceinline__ R low_term(const LowCell<R, NF>& x, int d, int q, R s_alpha) {
@@ -440,45 +431,6 @@ __device__ __forceinline__ R low_term(const LowCell<R, NF>& x, int d, int q, R s
         if (q == 1 + d) F += x.p;
     }
     return F - s_alpha * x.u[q];
-}
-
-// 4 resident blocks (64 registers, no spills): 0.336 -> 0.305 ms at 256^3; 3 blocks (80 registers) and a second plane of
-// prefetch (plane k + 2 in flight for a whole trip) both measured slower -- the kernel waits on L1/L2, not on DRAM latency
-#ifndef LOWUP_BLOCKS
-#define LOWUP_BLOCKS 4
-#endif
-template <typename R, int NF>
-__global__ void __launch_bounds__(256, LOWUP_BLOCKS) k_lowup(LowArgs<R> a, int seg_len) {
-    typedef Real<R> T;
-    R alpha[3];
-#pragma unroll
-    for (int d = 0; d < 3; ++d) alpha[d] = T::from_bits(a.diag->slot[a.slot].alpha_bits[d]);
-    const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y;
-    const int k0 = blockIdx.z * seg_len, k1 = min(a.nz, k0 + seg_len);
-    if (i >= a.nx || j >= a.ny || k0 >= k1) return;
-    const long long sx = 1, sy = a.nxp, sz = (long long)a.nxp * a.ny;
-    long long c = ((long long)k0 * a.ny + j) * a.nxp + i;
-    LowCell<R, NF> below, here, above, nb;
-    low_load<R, NF>(a, c, here);
-    low_load<R, NF>(a, k0 > 0 ? c - sz : c, below);
-    for (int k = k0; k < k1; ++k, c += sz) {
-        low_load<R, NF>(a, k < a.nz - 1 ? c + sz : c, above);
-        R acc[NF];
-        // sum over the two faces of a direction: (F^L_+ - F^L_-) = [ (F_p - alpha U_p) - (F_m + alpha U_m) ] / 2 + alpha U_c
-        _Pragma("unroll") for (int q = 0; q < NF; ++q)
-            acc[q] = R(0.5) * (low_term<R, NF>(above, 2, q, alpha[2]) - low_term<R, NF>(below, 2, q, -alpha[2])) + alpha[2] * here.u[q];
-        low_load<R, NF>(a, i < a.nx - 1 ? c + sx : c, nb);
-        _Pragma("unroll") for (int q = 0; q < NF; ++q) acc[q] += R(0.5) * low_term<R, NF>(nb, 0, q, alpha[0]) + alpha[0] * here.u[q];
-        low_load<R, NF>(a, i > 0 ? c - sx : c, nb);
-        _Pragma("unroll") for (int q = 0; q < NF; ++q) acc[q] -= R(0.5) * low_term<R, NF>(nb, 0, q, -alpha[0]);
-        low_load<R, NF>(a, j < a.ny - 1 ? c + sy : c, nb);
-        _Pragma("unroll") for (int q = 0; q < NF; ++q) acc[q] += R(0.5) * low_term<R, NF>(nb, 1, q, alpha[1]) + alpha[1] * here.u[q];
-        low_load<R, NF>(a, j > 0 ? c - sy : c, nb);
-        _Pragma("unroll") for (int q = 0; q < NF; ++q) acc[q] -= R(0.5) * low_term<R, NF>(nb, 1, q, -alpha[1]);
-        _Pragma("unroll") for (int q = 0; q < NF; ++q) a.UL[q * a.Np + c] = T::fma_(-a.lam, acc[q], here.u[q]);
-        below = here;
-        here = above;
-    }
 }
 
 // out = (A - B) / dt over the interior cells: L of the limited scheme for hydro_eval_rhs, from the limited Euler update
