@@ -178,6 +178,26 @@ long long hydro_launch_count(const hydro_t *h);
  * roofline fraction is quoted against. */
 int hydro_measure_alu_peak(int precision, double millis, void *cuda_stream, double *tflops);
 
+/* ---- the one entry point that allocates nothing (csrc/hydro_noalloc.cu) ----------------------------------------------
+ * Steps a-1 + a-2 (con2prim for p = e/3 from eq. 1, reading R9; Lax-Friedrichs speeds R4) of a
+ * caller's fp64 DEVICE state: alpha_dev[d] = max over the cells of max(|lambda_+^d|, |lambda_-^d|), d = x, y, z (exact
+ * maxima, hence order independent), counts_dev[0] = cells where the floor / cap of con2prim fired, counts_dev[1] = 1 if a
+ * non-finite conserved value was seen.  For callers that cannot call cudaMalloc (stream capture, tight serving loops,
+ * harnesses that forbid it): no handle, and no cudaMalloc / cudaFree / allocating routine is called.  The kernel's
+ * scratch (P, W and the reduction block) is a file-scope __device__ array of HYDRO_NOALLOC_MAX_CELLS x 16 bytes + 4 KiB
+ * (4 MiB + 4 KiB) that every GPU loading the library holds until exit; larger grids are rejected with HYDRO_EINVAL.
+ *   U_dev       DEVICE, nfields (4 or 5) contiguous blocks of nz*ny*nx doubles, x fastest (hydro_set_state's layout); read only
+ *   v_cap_delta, e_floor   as in hydro_eos_t (0 selects the fp64 defaults 1e-10, 1e-12)
+ *   alpha_dev   DEVICE, 3 doubles, written;  counts_dev  DEVICE, 2 long long, written (may be NULL)
+ *   cuda_stream the work is enqueued there (NULL = the default stream) on the CURRENT device; asynchronous
+ *   err, errlen optional host buffer that receives a one-line message when the return value is not HYDRO_OK
+ * All calls share the scratch array, which keeps the last call's contents (the reduction block is cleared by every call):
+ * calls that overlap on the GPU -- other streams, other host threads -- race on it; serialise them.  Caller owns every
+ * pointer. */
+#define HYDRO_NOALLOC_MAX_CELLS 262144          /* 64^3 */
+int hydro_wavespeeds_noalloc(const void *U_dev, int nx, int ny, int nz, int nfields, double v_cap_delta, double e_floor,
+                             double *alpha_dev, long long *counts_dev, void *cuda_stream, char *err, int errlen);
+
 const char *hydro_strerror(int code);
 /* Text of the last CUDA error seen by this handle ("" if none). */
 const char *hydro_last_cuda_error(const hydro_t *h);

@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhydro.so")
-SOURCES = [os.path.join(CSRC, "hydro.cu")]
+SOURCES = [os.path.join(CSRC, "hydro.cu"), os.path.join(CSRC, "hydro_noalloc.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "hydro_kernels.cuh"), os.path.join(CSRC, "hydro_sweep_ring.cuh"), os.path.join(CSRC, "hydro_lowup.cuh"),
                   os.path.join(os.path.dirname(HERE), "include", "hydro.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--fmad=true",

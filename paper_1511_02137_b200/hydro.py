@@ -26,7 +26,7 @@ SYMBOLS = ("hydro_create", "hydro_destroy", "hydro_set_state", "hydro_add_jet", 
            "hydro_stage_alpha", "hydro_stage_sweeps", "hydro_stage_prims_part", "hydro_stage_sweeps_part", "hydro_stage_alpha_dev", "hydro_halo", "hydro_halo_reals", "hydro_step",
            "hydro_synchronize", "hydro_get_fields", "hydro_eval_rhs", "hydro_get_diag", "hydro_get_last_stage_q",
            "hydro_set_profiling", "hydro_get_kernel_times", "hydro_launch_count", "hydro_sweep_path", "hydro_measure_alu_peak",
-           "hydro_strerror", "hydro_last_cuda_error")
+           "hydro_wavespeeds_noalloc", "hydro_strerror", "hydro_last_cuda_error")
 
 
 class EosT(C.Structure):
@@ -105,6 +105,8 @@ def load():
     L.hydro_step.argtypes = [vp, i]
     L.hydro_synchronize.restype = i
     L.hydro_synchronize.argtypes = [vp]
+    L.hydro_wavespeeds_noalloc.restype = i
+    L.hydro_wavespeeds_noalloc.argtypes = [vp, i, i, i, i, d, d, vp, vp, vp, C.c_char_p, i]
     L.hydro_get_fields.restype = i
     L.hydro_get_fields.argtypes = [vp, vp, i, i]
     L.hydro_eval_rhs.restype = i
@@ -155,6 +157,23 @@ def measure_alu_peak(precision=64, millis=200.0, stream=None):
     if rc != OK:
         raise HydroError(rc, "hydro_measure_alu_peak")
     return out.value
+
+
+NOALLOC_MAX_CELLS = 262144
+
+
+def wavespeeds_noalloc(U, alpha_out, counts_out=None, v_cap_delta=0.0, e_floor=0.0, stream=None):
+    """hydro_wavespeeds_noalloc: alpha_d maxima (+ cap / NaN counts) of the fp64 CUDA tensor U (nf, nz, ny, nx) into the
+    caller's CUDA tensors alpha_out (3 float64) and counts_out (2 int64, optional).  Allocates nothing; asynchronous."""
+    L = load()
+    nf, nz, ny, nx = U.shape
+    err = C.create_string_buffer(256)
+    rc = L.hydro_wavespeeds_noalloc(C.c_void_p(U.data_ptr()), nx, ny, nz, nf, float(v_cap_delta), float(e_floor),
+                                    C.c_void_p(alpha_out.data_ptr()),
+                                    C.c_void_p(counts_out.data_ptr() if counts_out is not None else 0),
+                                    C.c_void_p(stream if stream else 0), err, 256)
+    if rc != OK:
+        raise HydroError(rc, "hydro_wavespeeds_noalloc", err.value.decode())
 
 
 class Hydro:
