@@ -102,6 +102,9 @@ __host__ __device__ constexpr int ring_smem_bytes(int nf, int out, int esz, int 
             + RING_SUB) * esz                              // one tile of zeros
            + 64;                                           // mbarriers
 }
+#ifndef RING_LIM_X_PAIRS
+#define RING_LIM_X_PAIRS 1
+#endif
 #ifndef RING_F64_BLOCKS
 #define RING_F64_BLOCKS 3
 #endif
@@ -409,6 +412,47 @@ __device__ __noinline__ int theta_row(int r, const R* st, const R* stp, const R*
     }
     th[o] = theta;
     return theta < R(1) ? 1 : 0;
+}
+
+// x sweeps: theta of the faces of chunk rows r0 (even) and r0 + 1 together.  In the swizzled x tiles a lane's march cells
+// r0, r0 + 1 share one 16-byte chunk, and a warp's 8-byte loads of ONE row are 2-way bank conflicted whatever the swizzle
+// (all lanes read the same half of their 16-byte chunk: ncu counts 48-53e6 conflicts in 102-111e6 shared-memory wavefronts
+// of the limiter x kernels and 0.9-1.0 short-scoreboard stall cycles per issued instruction, against 0.44 in y/z), while
+// 16-byte loads of a row PAIR are conflict-free: 12 loads (8 of them pairs) instead of 24 for the two faces.
+template <int NF>
+__device__ __noinline__ int theta_rows2_x(int r0, const double* st, const double* stp, const double* xc_all, double* th, int lane,
+                                          int cm, int nd, double k3lam) {
+    const int sw = (lane >> 1) & 3;
+    const int o2 = lane * 8 + (((r0 >> 1) ^ sw) << 1);                     // rows r0, r0 + 1 of this lane
+    double2 c[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) c[q] = *reinterpret_cast<const double2*>(xc_all + q * RING_SUB + o2);
+    // U^L of the cells i0 = cm + r0 - 4, i0 + 1 (rows (r0 + 4) & 7, + 1: one pair) and i0 + 2 (row (r0 + 6) & 7)
+    const int i0 = cm + r0 - 4;
+    const double* sa = r0 < 4 ? stp : st;
+    const int oa = lane * 8 + (((((r0 + 4) & 7) >> 1) ^ sw) << 1);
+    const double* sc = r0 < 2 ? stp : st;
+    const int oc = lane * 8 + (((((r0 + 6) & 7) >> 1) ^ sw) << 1);
+    double2 ua[4];
+    double uc[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        ua[q] = *reinterpret_cast<const double2*>(sa + q * RING_SUB + oa);
+        uc[q] = sc[q * RING_SUB + oc];
+    }
+    const double A[4] = {ua[0].x, ua[1].x, ua[2].x, ua[3].x}, B[4] = {ua[0].y, ua[1].y, ua[2].y, ua[3].y};
+    const double c0[4] = {c[0].x, c[1].x, c[2].x, c[3].x}, c1[4] = {c[0].y, c[1].y, c[2].y, c[3].y};
+    double t0 = 1.0, t1 = 1.0;
+    if (i0 >= 0 && i0 <= nd - 1) { const double t = theta_cell<double>(A, c0, -k3lam); t0 = t < t0 ? t : t0; }
+    if (i0 + 1 >= 0 && i0 + 1 <= nd - 1) {
+        double t = theta_cell<double>(B, c0, k3lam);
+        t0 = t < t0 ? t : t0;
+        t = theta_cell<double>(B, c1, -k3lam);
+        t1 = t < t1 ? t : t1;
+    }
+    if (i0 + 2 >= 0 && i0 + 2 <= nd - 1) { const double t = theta_cell<double>(uc, c1, k3lam); t1 = t < t1 ? t : t1; }
+    *reinterpret_cast<double2*>(th + o2) = make_double2(t0, t1);
+    return (t0 < 1.0 ? 1 : 0) + (t1 < 1.0 ? 1 : 0);
 }
 
 template <typename R, int ORDER, int LIM, int DIR, int OUT, int NF>
@@ -726,8 +770,13 @@ k_sweep_ring(const __grid_constant__ RingMaps maps, const RingArgs a) {
             const R k3 = (R)a.k3lam;
             int n0 = 0, n1 = 0;
             if (f < 4) {                                            // warp f: the faces of rows 2f and 2f + 1
-                n0 = theta_row<DIR, NF, R>(2 * f, ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3);
-                n1 = theta_row<DIR, NF, R>(2 * f + 1, ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3);
+                if constexpr (DIR == 0 && sizeof(R) == 8 && RING_LIM_X_PAIRS) {
+                    n0 = theta_rows2_x<NF>(2 * f, (const double*)ul_cur, (const double*)ul_prev, (const double*)xcm, (double*)tht,
+                                           lane, cm, nd, (double)k3);   // both faces; x sweep: one ownership test serves both
+                } else {
+                    n0 = theta_row<DIR, NF, R>(2 * f, ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3);
+                    n1 = theta_row<DIR, NF, R>(2 * f + 1, ul_cur, ul_prev, xcm, tht, lane, cm, nd, k3);
+                }
             }
             if (n0 | n1) {                                          // rare: only now look at ownership (z-slabs)
                 const int il = cm + 2 * f - 4;                      // faces of rows 2f, 2f+1: lower cells il, il + 1
